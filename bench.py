@@ -1,0 +1,281 @@
+#!/usr/bin/env python
+"""bench.py -- throughput of the MD two-electron-integral hot path on BASELINE.json configs[1].
+
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--impl ours|reference] [--variants]
+
+A step is one pass of the whole hot path (pair setup, Boys, Hermite Coulomb tensor, both
+Hermite->AO contractions, solid-harmonic transform, store) over one batch: the 200,000
+independent (dd|dd) shell quartets of BASELINE.json configs[1], K = 3 per shell, solid-harmonic
+output, seed 0 (+rank).  Prints ONE JSON line.  With N > 1 (torchrun)
+every rank runs its own batch (quartets are independent: no data-path collective; weak scaling).
+"""
+import argparse
+import json
+import os
+import subprocess
+import sys
+import threading
+import time
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+sys.path.insert(0, ROOT)
+
+METRIC = "FP64 % of B200 peak and shell-quartets/s per (la lb|lc ld) class and K"
+UNIT = "shell-quartets/s"
+NQ = 200_000
+FP64_PEAK_DERIVED_TFLOPS = 148 * 64 * 2 * 1.965e9 / 1e12      # 37.2
+
+
+def workload(K, rank=0, n=NQ):
+    from paper_2405_01834_b200 import workloads as W
+    w = W.config2(K=K, n=n)
+    if rank:
+        w = W.independent_quartets(f"cfg2_dddd_K{K}_r{rank}", (2, 2, 2, 2), (K,) * 4, n, (0.05, 50.0), (-5.0, 5.0), rank)
+    return w
+
+
+def workload_name(K, pure, n=NQ):
+    return (f"BASELINE configs[1]: (dd|dd) FP64, K={K} per shell, {n} independent quartets, centers U[-5,5]^3, "
+            f"zeta log-uniform [0.05,50], {'solid-harmonic' if pure else 'Cartesian'} output, seed 0")
+
+
+class ClockSampler:
+    """nvidia-smi clocks / throttle reasons sampled every 200 ms while the timed region runs."""
+    Q = ("clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.hw_slowdown,clocks_event_reasons.hw_thermal_slowdown,"
+         "clocks_event_reasons.sw_thermal_slowdown,clocks_event_reasons.sw_power_cap")
+
+    def __init__(self, index):
+        self.lines, self.proc, self.index = [], None, index
+
+    def __enter__(self):
+        try:
+            self.proc = subprocess.Popen(["nvidia-smi", "-i", str(self.index), f"--query-gpu={self.Q}",
+                                          "--format=csv,noheader,nounits", "-lms", "200"],
+                                         stdout=subprocess.PIPE, stderr=subprocess.DEVNULL, text=True)
+            self.t = threading.Thread(target=lambda: self.lines.extend(self.proc.stdout), daemon=True)
+            self.t.start()
+        except OSError:
+            self.proc = None
+        return self
+
+    def __exit__(self, *a):
+        if self.proc:
+            self.proc.terminate()
+            self.t.join(timeout=2)
+
+    def summary(self):
+        sm, mx, reasons = [], [], set()
+        names = ["hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"]
+        for ln in self.lines:
+            f = [x.strip() for x in ln.split(",")]
+            if len(f) < 7:
+                continue
+            try:
+                sm.append(float(f[0])); mx.append(float(f[1]))
+            except ValueError:
+                continue
+            for nm, v in zip(names, f[3:7]):
+                if v.lower().startswith("active"):
+                    reasons.add(nm)
+        sm.sort()
+        return {"sm_mhz": sm[len(sm) // 2] if sm else None, "sm_max_mhz": max(mx) if mx else None,
+                "reasons": sorted(reasons), "samples": len(sm)}
+
+
+def time_steps(fn, steps, warmup, flush, dist_barrier):
+    """W warm-ups, then K steps timed with CUDA events on the launching (current) stream; L2 is
+    flushed between steps (outside the events).  Returns the summed device ms over the K steps."""
+    import torch
+    for _ in range(warmup):
+        fn()
+    torch.cuda.synchronize()
+    dist_barrier()
+    torch.cuda.synchronize()
+    ev = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)) for _ in range(steps)]
+    for e0, e1 in ev:
+        flush.fill_(1.0)                      # 256 MiB write > 126 MB L2
+        e0.record()
+        fn()
+        e1.record()
+    torch.cuda.synchronize()
+    dist_barrier()
+    return sum(e0.elapsed_time(e1) for e0, e1 in ev)
+
+
+def cpu_baseline(K, pure, nsample):
+    """The oracle as it stands, on this box's host cores, on the first nsample quartets."""
+    import numpy as np
+    import oracle
+    w = workload(K)
+    sel = np.arange(nsample)
+    ia, ib, ic, id_ = w.shell_indices(sel)
+    oracle.eri4(w.a.astuple(), w.b.astuple(), w.c.astuple(), w.d.astuple(), ia[:8], ib[:8], ic[:8], id_[:8], pure)
+    t = time.perf_counter()
+    oracle.eri4(w.a.astuple(), w.b.astuple(), w.c.astuple(), w.d.astuple(), ia, ib, ic, id_, pure)
+    dt = time.perf_counter() - t
+    return {"value": nsample / dt, "unit": UNIT, "cores": oracle.max_threads(), "kind": "oracle",
+            "sample": f"first {nsample} of the {NQ} quartets, {dt:.1f} s, gcc -O2 OpenMP over quartets"}, dt
+
+
+def run_reference(args):
+    rank = int(os.environ.get("RANK", "0"))
+    if rank != 0:
+        return
+    K, pure = 3, True
+    nsample = 4000
+    vals = []
+    for _ in range(args.warmup):
+        cpu_baseline(K, pure, 200)
+    for _ in range(args.steps):
+        cb, dt = cpu_baseline(K, pure, nsample)
+        vals.append((cb, dt))
+    tot = sum(dt for _, dt in vals)
+    v = nsample * len(vals) / tot
+    cb = dict(vals[-1][0]); cb["value"] = v
+    print(json.dumps({"impl": "reference", "metric": METRIC, "value": v, "unit": UNIT, "n_gpus": args.gpus,
+                      "steps": args.steps, "warmup": args.warmup, "ms_per_step": 1e3 * tot / len(vals),
+                      "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f64",
+                      "data": "synthetic", "config": {"workload": workload_name(K, pure), "sample_per_step": nsample},
+                      "cpu_baseline": cb,
+                      "e2e": {"value": v, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0}}))
+
+
+def measure_variant(dw, w, K, pure, steps, warmup, flush, barrier):
+    from paper_2405_01834_b200 import engine, workloads as W
+    out = dw.alloc_out(pure)
+    ms = time_steps(lambda: dw.run(pure, out), steps, warmup, flush, barrier)
+    flops = W.flops_model(2, 2, 2, 2, K * K, K * K, pure)
+    return {"K": K, "pure": pure, "ms_per_step": ms / steps, "quartets_per_s": w.nquartets * steps / (ms * 1e-3),
+            "model_flop_per_quartet": flops, "model_tflops": flops * w.nquartets * steps / (ms * 1e-3) / 1e12,
+            "variant": {1: "generic", 2: "fused"}.get(engine.md_last_variant(), "?"),
+            "launches_per_step": engine.md_last_launch_count(), "out_bytes": out.numel() * 8}
+
+
+def run_ours(args):
+    import numpy as np
+    import torch
+    import torch.distributed as dist
+    from paper_2405_01834_b200 import build, engine, workloads as W
+
+    rank = int(os.environ.get("RANK", "0"))
+    local = int(os.environ.get("LOCAL_RANK", "0"))
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py needs a CUDA device: the engine has no CPU fallback")
+    build.build()
+    torch.cuda.set_device(local)
+    if world > 1:
+        dist.init_process_group("nccl", device_id=torch.device("cuda", local))
+    barrier = (lambda: dist.barrier()) if world > 1 else (lambda: None)
+    engine.md_init()
+    flush = torch.empty(256 << 20, dtype=torch.uint8, device="cuda")
+
+    K, pure = 3, True
+    w = workload(K, rank)
+    dw = engine.DeviceWorkload(w)
+    with ClockSampler(local) as cs:
+        head = measure_variant(dw, w, K, pure, args.steps, args.warmup, flush, barrier)
+    clocks = cs.summary()
+    ms_total = head["ms_per_step"] * args.steps
+    if world > 1:
+        t = torch.tensor([ms_total], dtype=torch.float64, device="cuda")
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+        ms_total = float(t.item())
+    value = world * w.nquartets * args.steps / (ms_total * 1e-3)
+
+    # end to end: the host-buffer C-ABI call, pinned host memory, copies inside the timed region
+    esteps = max(1, min(args.steps, 3))
+    host_out = torch.empty(w.nquartets * w.nout(pure), dtype=torch.float64).pin_memory()
+    pinned = [torch.as_tensor(x).pin_memory() for s in (w.a, w.b, w.c, w.d) for x in (s.center, s.exps, s.coefs)]
+    hq = torch.as_tensor(w.quartet_idx).pin_memory()
+
+    class _S:
+        pass
+    hs = []
+    for i, s in enumerate((w.a, w.b, w.c, w.d)):
+        o = _S(); o.l, o.K, o.n = s.l, s.K, s.n
+        o.center, o.exps, o.coefs = pinned[3 * i: 3 * i + 3]
+        hs.append(o)
+    h2d = sum(t.numel() * t.element_size() for t in pinned) + hq.numel() * 4
+    d2h = host_out.numel() * 8
+
+    def e2e_step():
+        engine.md_eri4_host(hs[0], hs[1], hs[2], hs[3], None, None, hq, w.nquartets, pure, host_out,
+                            nbra=w.nbra, nket=w.nket)
+    e2e_step()
+    torch.cuda.synchronize(); barrier()
+    t0 = time.perf_counter()
+    for _ in range(esteps):
+        e2e_step()
+    torch.cuda.synchronize(); barrier()
+    e2e_s = time.perf_counter() - t0
+    if world > 1:
+        t = torch.tensor([e2e_s], dtype=torch.float64, device="cuda")
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+        e2e_s = float(t.item())
+    e2e_val = world * w.nquartets * esteps / e2e_s
+
+    line = {"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
+            "ms_per_step": ms_total / args.steps, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
+            "dtype": "f64", "data": "synthetic",
+            "config": {"workload": workload_name(K, pure), "quartets_per_gpu": w.nquartets, "class": "(dd|dd)", "K": K,
+                       "output": "solid", "structure": "independent quartets (2 fresh pairs per quartet)",
+                       "l2": "256 MiB flush write between timed steps", "kernel_variant": head["variant"]},
+            "clocks": clocks,
+            "e2e": {"value": e2e_val, "unit": UNIT, "h2d_bytes_per_step": h2d, "d2h_bytes_per_step": d2h,
+                    "steps": esteps, "api": "md_eri4_host, pinned host buffers"},
+            "gpu_launches": head["launches_per_step"] * args.steps}
+
+    if rank == 0:
+        # roofline of the step (one fused kernel, or pair setup + quartet kernel): algorithmic flops of the
+        # Table I model over the CUDA-event duration, against the FP64 DFMA peak.
+        dfma_tf, _ = engine.md_fp64_peak(0, 0.5)
+        dmma_tf, _ = engine.md_fp64_peak(1, 0.3)
+        achieved = head["model_tflops"]
+        line["roofline"] = {"bound": "alu", "achieved": achieved, "peak": FP64_PEAK_DERIVED_TFLOPS, "unit": "TFLOP/s",
+                            "frac": achieved / FP64_PEAK_DERIVED_TFLOPS, "traffic": None,
+                            "peak_source": "derived: 148 SM x 64 DFMA/clk x 2 x 1.965 GHz (DESIGN.md)",
+                            "peak_measured_dfma_loop": dfma_tf, "peak_measured_dmma_m8n8k4_loop": dmma_tf,
+                            "frac_of_measured_dfma": achieved / dfma_tf if dfma_tf else None,
+                            "algorithmic_flop_per_quartet": head["model_flop_per_quartet"],
+                            "kernel": "md_eri4 step (all launches of the call)",
+                            "hbm_gbs_algorithmic": (head["out_bytes"] + h2d) / (head["ms_per_step"] * 1e-3) / 1e9}
+        try:
+            peaks = json.load(open(os.path.join(ROOT, "MEASURED_PEAKS.json")))
+            line["roofline"]["hbm_peak_gbs_measured"] = peaks.get("hbm_gbs")
+        except (OSError, ValueError):
+            line["roofline"]["hbm_peak_gbs_measured"] = None
+        if world == 1:
+            cb, _ = cpu_baseline(K, pure, args.cpu_sample)
+            line["cpu_baseline"] = cb
+            if args.variants:
+                extra = []
+                for k2, p2 in ((1, True), (1, False), (3, False)):
+                    w2 = workload(k2)
+                    dw2 = engine.DeviceWorkload(w2)
+                    extra.append(measure_variant(dw2, w2, k2, p2, args.steps, args.warmup, flush, barrier))
+                    del dw2
+                line["variants"] = [head] + extra
+        print(json.dumps(line))
+    if world > 1:
+        dist.destroy_process_group()
+
+
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=5)
+    ap.add_argument("--warmup", type=int, default=3)
+    ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    ap.add_argument("--variants", action="store_true", help="also time K=1 and Cartesian output")
+    ap.add_argument("--cpu-sample", type=int, default=8000)
+    args = ap.parse_args()
+    args.warmup = max(args.warmup, 3) if args.impl == "ours" else args.warmup
+    if args.impl == "reference":
+        run_reference(args)
+    else:
+        run_ours(args)
+
+
+if __name__ == "__main__":
+    main()

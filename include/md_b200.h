@@ -1,0 +1,168 @@
+/*
+ * md_b200.h -- C ABI of the B200-native McMurchie-Davidson two-electron integral engine.
+ *
+ * The library evaluates, in FP64 on one sm_100a GPU, batches of
+ *   4-center integrals (ab|cd)   PAPER.md:43-45, Eq. 3
+ *   3-center integrals (ab|X)    PAPER.md:39-41, Eq. 2, read as (ab|X) = [X|ab] (reading S5)
+ * over contracted Cartesian Gaussian shells (Eqs. 1 and 4) by the
+ * McMurchie-Davidson scheme of PAPER.md section II (Eqs. 5-26): primitive-pair Hermite
+ * expansion E/H, Boys function, Hermite Coulomb tensor [r]^(0), the two Hermite->AO
+ * contractions, and the Cartesian->solid-harmonic transform.  The call shape follows the
+ * paper's Listing IV.1: lists of bra and ket shell pairs, a caller-owned
+ * target buffer, asynchronous on a CUDA stream.
+ *
+ * Conventions common to every call
+ * --------------------------------
+ * Memory.  md_eri4 / md_eri3 take DEVICE pointers for every array (shell data, index lists,
+ *   output).  md_eri4_host / md_eri3_host take HOST pointers for every array and perform
+ *   the host<->device copies themselves (they synchronise the stream before returning).
+ *   The structs themselves are always host memory.  The caller owns every buffer; the
+ *   library never frees or reallocates caller memory.  Scratch (per-pair Hermite data) is a
+ *   grow-only device cache owned by the library unless md_set_workspace gives it a buffer.
+ * Asynchrony.  md_eri4 / md_eri3 enqueue work on `cuda_stream` (a cudaStream_t cast to
+ *   void*; NULL = the legacy default stream) and return without synchronising, as the
+ *   paper's compute() does.  Growing the internal workspace synchronises.
+ * Errors.  Return 0 (MD_OK) or a negative code; nothing is written to `out` on an argument
+ *   error.  No exception crosses the ABI.  md_last_cuda_error() returns the CUDA runtime's
+ *   text for the most recent MD_ECUDA.
+ * Normalisation.  None is applied (the paper states none): a primitive is exactly
+ *   PAPER.md Eq. 1 times coefs[k]; every Cartesian component of a shell uses the same coefs.
+ * Component order inside a shell of angular momentum l (0 <= l <= MD_MAX_L):
+ *   Cartesian (pure = 0): ax = l..0, ay = l-ax..0, az = l-ax-ay  (xx xy xz yy yz zz), (l+1)(l+2)/2.
+ *   Solid     (pure = 1): m = -l..+l, Racah-normalised real solid harmonics without
+ *     Condon-Shortley phase (S_1,{-1,0,1} = y,z,x; S_20 = zz-(xx+yy)/2), 2l+1 components
+ *     (Eqs. 16-17; coefficient formula in DESIGN.md reading O2).
+ * Output layouts (n_a.. = component counts, N_ab = n_a n_b, N_cd = n_c n_d):
+ *   MD_LAYOUT_QUARTET_MAJOR  out[q*N_ab*N_cd + ((a*n_b + b)*n_c + c)*n_d + d], q = quartet number.
+ *   MD_LAYOUT_PAPER          the paper's V[ij,ab,cd,kl], column-major, bra pair ij fastest
+ *                            (PAPER.md:198): out[ij + nbra*(ab + N_ab*(cd + N_cd*kl))];
+ *                            only for the full bra x ket product (quartet_idx == NULL).
+ *   3-center: the same with d absent: [t][a][b][mX].
+ */
+#ifndef MD_B200_H
+#define MD_B200_H
+
+#include <stddef.h>
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+#define MD_MAX_L 6            /* s..i */
+#define MD_MAX_K 16           /* contraction degree per shell accepted by the engine */
+
+#define MD_OK          0
+#define MD_EINVAL    (-1)     /* l outside 0..MD_MAX_L, K outside 1..MD_MAX_K, n < 0, NULL array, bad flag */
+#define MD_ECAPACITY (-2)     /* out_capacity_elems smaller than the result */
+#define MD_ECUDA     (-3)     /* CUDA runtime error (allocation, launch, copy) */
+#define MD_ENOMEM    (-4)     /* caller-set workspace too small for this call */
+
+#define MD_LAYOUT_QUARTET_MAJOR 0
+#define MD_LAYOUT_PAPER         1
+
+/* Homogeneous shell batch: n shells that share l and K (pairs are grouped by
+ * l and contraction degree).  Arrays are row-major. */
+typedef struct {
+    int32_t l;               /* angular momentum, 0..MD_MAX_L                           */
+    int32_t K;               /* contraction degree, 1..MD_MAX_K (Eq. 4)        */
+    int64_t n;               /* number of shells                                        */
+    const double *center;    /* [n][3]  bohr                                            */
+    const double *exps;      /* [n][K]  zeta_k > 0                                      */
+    const double *coefs;     /* [n][K]  c_k, already including any normalisation        */
+} md_shells;
+
+/* Pair batch: pair i = (a[idx[2i]], b[idx[2i+1]]); idx == NULL means pair i = (a[i], b[i])
+ * and then npairs <= min(a.n, b.n).  One (la, lb, Ka, Kb) class per batch. */
+typedef struct {
+    md_shells a, b;
+    int64_t npairs;
+    const int32_t *idx;      /* [npairs][2] or NULL */
+} md_pairs;
+
+/*
+ * (ab|cd) for nquartets quartets (Eq. 3 through Eqs. 7, 19, 21-26).
+ *   quartet q = (bra pair quartet_idx[2q], ket pair quartet_idx[2q+1]);
+ *   quartet_idx == NULL: the full product, q = ij*ket->npairs + kl, and nquartets must equal
+ *   bra->npairs * ket->npairs.
+ * Any order of l and K between the four shells is accepted.  Index lists are trusted (no
+ * range check on the device).  out must hold md_eri4_out_elems(...) doubles.
+ */
+int md_eri4(const md_pairs *bra, const md_pairs *ket,
+            int64_t nquartets, const int32_t *quartet_idx,
+            int pure, int layout,
+            double *out, int64_t out_capacity_elems, void *cuda_stream);
+
+/*
+ * (ab|X) for ntriplets triplets: the ket is the single shell X expanded about its own
+ * centre with the one-centre coefficients of PAPER.md Eqs. 6, 8, 11, 12 (q = zeta_X, Q = X).
+ *   triplet t = (bra pair triplet_idx[2t], shell X triplet_idx[2t+1]); NULL = full product,
+ *   t = ij*X->n + x.
+ */
+int md_eri3(const md_pairs *bra, const md_shells *X,
+            int64_t ntriplets, const int32_t *triplet_idx,
+            int pure, int layout,
+            double *out, int64_t out_capacity_elems, void *cuda_stream);
+
+/* Host-buffer forms: every array pointer (inside the structs too) is HOST memory.  The call
+ * copies inputs to the device, runs the same kernels, copies the result back into `out`
+ * and synchronises `cuda_stream` before returning. */
+int md_eri4_host(const md_pairs *bra, const md_pairs *ket,
+                 int64_t nquartets, const int32_t *quartet_idx,
+                 int pure, int layout,
+                 double *out, int64_t out_capacity_elems, void *cuda_stream);
+int md_eri3_host(const md_pairs *bra, const md_shells *X,
+                 int64_t ntriplets, const int32_t *triplet_idx,
+                 int pure, int layout,
+                 double *out, int64_t out_capacity_elems, void *cuda_stream);
+
+/* Number of doubles the result occupies (negative error code on bad arguments). */
+int64_t md_eri4_out_elems(int la, int lb, int lc, int ld, int pure, int64_t nquartets);
+int64_t md_eri3_out_elems(int la, int lb, int lX, int pure, int64_t ntriplets);
+
+/* Scratch the library needs for a call with these shapes, in bytes (per-pair Hermite data,
+ * PAPER.md:202 "{G, H[ab,p]}[ij,K_b]").  Classes served by a fused kernel need none. */
+int64_t md_eri4_workspace_bytes(const md_pairs *bra, const md_pairs *ket, int64_t nquartets,
+                                int list_mode, int pure);
+int64_t md_eri3_workspace_bytes(const md_pairs *bra, const md_shells *X, int64_t ntriplets,
+                                int list_mode, int pure);
+
+/* Give the library a caller-owned DEVICE scratch buffer (ptr == NULL returns to the internal
+ * grow-only cache).  With a caller buffer a call that needs more returns MD_ENOMEM. */
+int md_set_workspace(void *device_ptr, size_t bytes);
+
+/* Kernel-variant control, for measurement:
+ *   MD_VARIANT_AUTO    the measured-best variant per class (default)
+ *   MD_VARIANT_GENERIC the runtime-l kernel chain (pair setup + quartet kernel) for every class
+ *   MD_VARIANT_FUSED   the compile-time-l fused kernel where one exists, else generic  */
+#define MD_VARIANT_AUTO    0
+#define MD_VARIANT_GENERIC 1
+#define MD_VARIANT_FUSED   2
+int md_set_variant(int variant);
+/* Which variant the last md_eri4/md_eri3 call used (MD_VARIANT_GENERIC or MD_VARIANT_FUSED),
+ * and how many kernels it launched. */
+int md_last_variant(void);
+int md_last_launch_count(void);
+
+/* One-time initialisation (Boys table, component tables) on the current device.  Called
+ * implicitly by the first compute call; exposed so that timing can exclude it. */
+int md_init(void);
+
+/* Boys function F_m(T), m = 0..mmax <= 4*MD_MAX_L, for n values of T (device pointers;
+ * out is [n][mmax+1]); the device routine the integral kernels use (Eq. 22). */
+int md_boys(int mmax, int64_t n, const double *T, double *out, void *cuda_stream);
+
+/* Measurement helper (not on the hot path): best achieved FP64 rate, in TFLOP/s, of a pure
+ * issue loop running for about seconds_x10/10 s on the current device.
+ *   kind 0: DFMA (vector pipe), 1: DMMA mma.sync.m8n8k4.f64, 2: DMMA mma.sync.m16n8k8.f64.
+ * tflops and ms_out (duration of the best launch; may be NULL) are HOST pointers.  Synchronous. */
+int md_fp64_peak(int kind, int seconds_x10, double *tflops, double *ms_out);
+
+const char *md_strerror(int code);
+const char *md_last_cuda_error(void);
+int md_version(void);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* MD_B200_H */

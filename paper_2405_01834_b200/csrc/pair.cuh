@@ -1,0 +1,173 @@
+// pair.cuh -- step S1 of the hot path for the runtime-l kernel chain: primitive-pair setup.
+//
+// For every shell pair (a,b) of a pair batch and every primitive pair (ka,kb) this kernel
+// writes one record of `stride` doubles ("{G, H[ab,p]}[ij,K_b]" stored
+// contiguously per pair and primitive):
+//   rec[0]    = p = zeta_a + zeta_b
+//   rec[1..3] = P = (zeta_a A + zeta_b B)/p
+//   rec[4 + p~*N_ab + ab] = H[p~][ab]
+// with H the Hermite->AO matrix of PAPER.md Eqs. 7 and 17,
+//   Cartesian: H[p~][ab]   = c_a c_b E^{t}_{ax bx} E^{u}_{ay by} E^{v}_{az bz}
+//   solid    : H[p~][mamb] = sum_{a,b} C^{la}_{ma,a} C^{lb}_{mb,b} H[p~][ab]   (Eq. 17)
+// stored p~-major so that both Hermite->AO contractions read one contiguous row per Hermite
+// index.  For the ket batch the factor (-1)^{|q~|} of Eq. 19 is folded in (ket_sign = 1).
+// A one-centre batch (3-center X, Eqs. 6, 8, 11, 12) is the same recursion with
+// zeta_b = 0, c_b = 1, B = A (Eq. 8 is Eq. 9 at P = A; reading G2).
+#pragma once
+#include "common.cuh"
+
+namespace mdb {
+
+// One Cartesian axis of the two-centre expansion, E[(i*(lb+1)+j)*nt + t], nt = la+lb+1:
+//   E^0_00 = exp(-za zb xab^2/p)                                        (Eq. 13)
+//   E^t_{i,j+1} = E^{t-1}_{ij}/(2p) + (P-B) E^t_{ij} + (t+1) E^{t+1}_{ij}   (Eq. 10), at i = 0
+//   E^t_{i+1,j} = E^{t-1}_{ij}/(2p) + (P-A) E^t_{ij} + (t+1) E^{t+1}_{ij}   (Eq. 9),  every j
+//   E^t_{ij} = 0 outside 0 <= t <= i+j                                  (Eq. 14)
+__device__ inline void hermite_e_axis(int la, int lb, double za, double zb, double xab, double *E) {
+    const int nt = la + lb + 1;
+    const double p = za + zb, h = 0.5 / p;
+    const double xpa = -zb * xab / p, xpb = za * xab / p;
+    for (int k = 0; k < (la + 1) * (lb + 1) * nt; ++k) E[k] = 0.0;
+    E[0] = exp(-za * zb / p * xab * xab);
+    for (int j = 0; j < lb; ++j) {                       // row i = 0: raise j
+        const double *src = E + j * nt;
+        double *dst = E + (j + 1) * nt;
+        for (int t = 0; t <= j + 1; ++t) {
+            double v = xpb * src[t];
+            if (t > 0) v += h * src[t - 1];
+            if (t < j) v += (t + 1) * src[t + 1];
+            dst[t] = v;
+        }
+    }
+    for (int i = 0; i < la; ++i)                         // raise i for every j
+        for (int j = 0; j <= lb; ++j) {
+            const double *src = E + (i * (lb + 1) + j) * nt;
+            double *dst = E + ((i + 1) * (lb + 1) + j) * nt;
+            for (int t = 0; t <= i + j + 1; ++t) {
+                double v = xpa * src[t];
+                if (t > 0) v += h * src[t - 1];
+                if (t < i + j) v += (t + 1) * src[t + 1];
+                dst[t] = v;
+            }
+        }
+}
+
+struct PairSetupArgs {
+    PairView pv;
+    int pure;
+    int ket_sign;            // fold (-1)^{|q~|} (Eq. 19) into H
+    int pchunk;              // Hermite rows per shared-memory chunk of the solid transform
+    long long stride;        // doubles per (pair, primitive) record
+    double *rec;             // [npairs][Ka*Kb][stride]
+};
+
+// One CTA per (pair, primitive pair).  Shared memory: 3 axis tables + the stage-A buffer.
+__global__ void __launch_bounds__(128) pair_setup_kernel(PairSetupArgs g) {
+    extern __shared__ double sm[];
+    const PairView &pv = g.pv;
+    const int la = pv.a.l, lb = pv.single ? 0 : pv.b.l;
+    const int Ka = pv.a.K, Kb = pv.single ? 1 : pv.b.K;
+    const int Lb = la + lb, nt = Lb + 1, nh = nherm(Lb);
+    const int esz = (la + 1) * (lb + 1) * nt;
+    double *E = sm;                     // [3][esz]
+    double *T1 = sm + 3 * esz;          // [pchunk][nca][nb_out]
+    __shared__ double hdr[5];           // p, P, coefficient
+
+    const long long rid = blockIdx.x;   // pair * Ka*Kb + prim
+    const long long ipair = rid / (Ka * Kb);
+    const int kp = (int)(rid % (Ka * Kb)), ka = kp / Kb, kb = kp % Kb;
+    long long ia = ipair, ib = ipair;
+    if (pv.idx) { ia = pv.idx[2 * ipair]; ib = pv.idx[2 * ipair + 1]; }
+
+    if (threadIdx.x < 3) {
+        const int ax = threadIdx.x;
+        double za = pv.a.exps[ia * Ka + ka], A = pv.a.center[3 * ia + ax];
+        double zb = 0.0, B = A;
+        if (!pv.single) { zb = pv.b.exps[ib * Kb + kb]; B = pv.b.center[3 * ib + ax]; }
+        hermite_e_axis(la, lb, za, zb, A - B, E + ax * esz);
+        double p = za + zb;
+        hdr[1 + ax] = (za * A + zb * B) / p;
+        if (ax == 0) {
+            hdr[0] = p;
+            hdr[4] = pv.a.coefs[ia * Ka + ka] * (pv.single ? 1.0 : pv.b.coefs[ib * Kb + kb]);
+        }
+    }
+    __syncthreads();
+    double *rec = g.rec + rid * g.stride;
+    if (threadIdx.x < 4) rec[threadIdx.x] = hdr[threadIdx.x];
+    const double coef = hdr[4];
+    const int nca = ncart(la), ncb = ncart(lb);
+    const uint32_t *ca = c_herm + nherm(la - 1), *cb = c_herm + nherm(lb - 1);   // component exponents
+    const double *Ex = E, *Ey = E + esz, *Ez = E + 2 * esz;
+    double *H = rec + 4;
+
+    if (!g.pure) {
+        const int nab = nca * ncb;
+        for (int e = threadIdx.x; e < nh * nab; e += blockDim.x) {
+            int ih = e / nab, ab = e % nab, a = ab / ncb, b = ab % ncb;
+            int t, u, v, ax, ay, az, bx, by, bz;
+            unpack_tuv(c_herm[ih], t, u, v);
+            unpack_tuv(ca[a], ax, ay, az);
+            unpack_tuv(cb[b], bx, by, bz);
+            double val = coef * Ex[(ax * (lb + 1) + bx) * nt + t] * Ey[(ay * (lb + 1) + by) * nt + u] *
+                         Ez[(az * (lb + 1) + bz) * nt + v];
+            if (g.ket_sign && ((t + u + v) & 1)) val = -val;
+            H[e] = val;
+        }
+        return;
+    }
+    if (pv.single) {
+        // One-centre solid harmonics (Hobson): S_lm(d/dA) e^{-z r_A^2} = (2z)^l S_lm(r_A) e^{-z r_A^2}, so
+        // only the Hermites of order exactly l appear, with coefficient C^l_{m,q~}/(2z)^l.  Writing the
+        // zeros exactly (instead of leaving Eq. 17's cancellation to rounding) keeps the result accurate
+        // relative to the small solid block (finding F1).
+        const int nsa = nsolid(la), nlow = nherm(la - 1);
+        const double *Ca = c_solid + solid_off(la);
+        double f = coef;
+        for (int i = 0; i < la; ++i) f *= 0.5 / hdr[0];
+        if (g.ket_sign && (la & 1)) f = -f;
+        for (int e = threadIdx.x; e < nh * nsa; e += blockDim.x) {
+            int ih = e / nsa, m = e % nsa;
+            H[e] = ih < nlow ? 0.0 : f * Ca[m * nca + (ih - nlow)];
+        }
+        return;
+    }
+    // Solid harmonics, Eq. 17, one index at a time, pchunk Hermite rows per pass:
+    //   stage A  T1[p~][a][mb] = sum_b C^{lb}[mb][b] E^{ab}_{p~}
+    //   stage B  H[p~][ma][mb] = coef * sum_a C^{la}[ma][a] T1[p~][a][mb]
+    const int nsa = nsolid(la), nsb = nsolid(lb);
+    const double *Ca = c_solid + solid_off(la), *Cb = c_solid + solid_off(lb);
+    for (int h0 = 0; h0 < nh; h0 += g.pchunk) {
+        const int hc = min(g.pchunk, nh - h0);
+        for (int e = threadIdx.x; e < hc * nca * nsb; e += blockDim.x) {
+            int ih = e / (nca * nsb), r = e % (nca * nsb), a = r / nsb, mb = r % nsb;
+            int t, u, v, ax, ay, az;
+            unpack_tuv(c_herm[h0 + ih], t, u, v);
+            unpack_tuv(ca[a], ax, ay, az);
+            double s = 0.0;
+            for (int b = 0; b < ncb; ++b) {
+                double c = Cb[mb * ncb + b];
+                if (c == 0.0) continue;
+                int bx, by, bz;
+                unpack_tuv(cb[b], bx, by, bz);
+                if (t > ax + bx || u > ay + by || v > az + bz) continue;
+                s += c * Ex[(ax * (lb + 1) + bx) * nt + t] * Ey[(ay * (lb + 1) + by) * nt + u] *
+                     Ez[(az * (lb + 1) + bz) * nt + v];
+            }
+            T1[e] = s;
+        }
+        __syncthreads();
+        for (int e = threadIdx.x; e < hc * nsa * nsb; e += blockDim.x) {
+            int ih = e / (nsa * nsb), r = e % (nsa * nsb), ma = r / nsb, mb = r % nsb;
+            const double *t1 = T1 + ih * nca * nsb + mb;
+            double s = 0.0;
+            for (int a = 0; a < nca; ++a) s += Ca[ma * nca + a] * t1[a * nsb];
+            s *= coef;
+            if (g.ket_sign && (c_herm[h0 + ih] >> 24 & 1)) s = -s;
+            H[(long long)(h0 + ih) * nsa * nsb + r] = s;
+        }
+        __syncthreads();
+    }
+}
+
+}  // namespace mdb

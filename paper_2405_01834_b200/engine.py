@@ -1,0 +1,251 @@
+"""Thin ctypes binding of include/md_b200.h.  Argument marshalling only: every step of the hot
+path runs in the CUDA library.  torch is used for device memory and streams.  There is no CPU
+fallback: if the library is missing this module raises at first use.
+"""
+import ctypes
+import os
+
+import numpy as np
+
+_HERE = os.path.dirname(os.path.abspath(__file__))
+LIB_PATH = os.path.join(_HERE, "libmdb200.so")
+
+MD_OK, MD_EINVAL, MD_ECAPACITY, MD_ECUDA, MD_ENOMEM = 0, -1, -2, -3, -4
+LAYOUT_QUARTET_MAJOR, LAYOUT_PAPER = 0, 1
+VARIANT_AUTO, VARIANT_GENERIC, VARIANT_FUSED = 0, 1, 2
+
+_dp = ctypes.POINTER(ctypes.c_double)
+_ip = ctypes.POINTER(ctypes.c_int32)
+
+
+class md_shells(ctypes.Structure):
+    _fields_ = [("l", ctypes.c_int32), ("K", ctypes.c_int32), ("n", ctypes.c_int64),
+                ("center", ctypes.c_void_p), ("exps", ctypes.c_void_p), ("coefs", ctypes.c_void_p)]
+
+
+class md_pairs(ctypes.Structure):
+    _fields_ = [("a", md_shells), ("b", md_shells), ("npairs", ctypes.c_int64), ("idx", ctypes.c_void_p)]
+
+
+SYMBOLS = ["md_eri4", "md_eri3", "md_eri4_host", "md_eri3_host", "md_eri4_out_elems", "md_eri3_out_elems",
+           "md_eri4_workspace_bytes", "md_eri3_workspace_bytes", "md_set_workspace", "md_set_variant",
+           "md_last_variant", "md_last_launch_count", "md_init", "md_boys", "md_fp64_peak", "md_strerror", "md_last_cuda_error",
+           "md_version"]
+
+_lib = None
+
+
+def lib():
+    """Load libmdb200.so (raises if it has not been built: there is no fallback path)."""
+    global _lib
+    if _lib is None:
+        if not os.path.exists(LIB_PATH):
+            raise RuntimeError(f"{LIB_PATH} is missing: run `python -m paper_2405_01834_b200.build` "
+                               "(the engine has no CPU fallback)")
+        L = ctypes.CDLL(LIB_PATH)
+        pp, ps = ctypes.POINTER(md_pairs), ctypes.POINTER(md_shells)
+        sig = [ctypes.c_int64, ctypes.c_void_p, ctypes.c_int, ctypes.c_int, ctypes.c_void_p, ctypes.c_int64,
+               ctypes.c_void_p]
+        for name, second in (("md_eri4", pp), ("md_eri3", ps), ("md_eri4_host", pp), ("md_eri3_host", ps)):
+            f = getattr(L, name)
+            f.argtypes = [pp, second] + sig
+            f.restype = ctypes.c_int
+        L.md_eri4_out_elems.argtypes = [ctypes.c_int] * 5 + [ctypes.c_int64]
+        L.md_eri4_out_elems.restype = ctypes.c_int64
+        L.md_eri3_out_elems.argtypes = [ctypes.c_int] * 4 + [ctypes.c_int64]
+        L.md_eri3_out_elems.restype = ctypes.c_int64
+        L.md_eri4_workspace_bytes.argtypes = [pp, pp, ctypes.c_int64, ctypes.c_int, ctypes.c_int]
+        L.md_eri4_workspace_bytes.restype = ctypes.c_int64
+        L.md_eri3_workspace_bytes.argtypes = [pp, ps, ctypes.c_int64, ctypes.c_int, ctypes.c_int]
+        L.md_eri3_workspace_bytes.restype = ctypes.c_int64
+        L.md_set_workspace.argtypes = [ctypes.c_void_p, ctypes.c_size_t]
+        L.md_set_variant.argtypes = [ctypes.c_int]
+        L.md_boys.argtypes = [ctypes.c_int, ctypes.c_int64, ctypes.c_void_p, ctypes.c_void_p, ctypes.c_void_p]
+        L.md_fp64_peak.argtypes = [ctypes.c_int, ctypes.c_int, _dp, _dp]
+        L.md_strerror.argtypes = [ctypes.c_int]
+        L.md_strerror.restype = ctypes.c_char_p
+        L.md_last_cuda_error.restype = ctypes.c_char_p
+        _lib = L
+    return _lib
+
+
+class MDError(RuntimeError):
+    def __init__(self, code):
+        L = lib()
+        msg = L.md_strerror(code).decode()
+        if code == MD_ECUDA:
+            msg += ": " + L.md_last_cuda_error().decode()
+        super().__init__(f"md_b200 error {code}: {msg}")
+        self.code = code
+
+
+def _check(code):
+    if code != MD_OK:
+        raise MDError(code)
+
+
+def _ptr(x):
+    """Raw address of a torch tensor (device or host) or a numpy array; None -> NULL."""
+    if x is None:
+        return None
+    if isinstance(x, np.ndarray):
+        return x.ctypes.data
+    return x.data_ptr()
+
+
+def _shells_struct(s):
+    """s: anything with .l .K .n .center .exps .coefs (arrays already on the wanted side)."""
+    return md_shells(int(s.l), int(s.K), int(s.n), _ptr(s.center), _ptr(s.exps), _ptr(s.coefs))
+
+
+def _pairs_struct(a, b, idx, npairs=None):
+    n = (idx.shape[0] if idx is not None else min(a.n, b.n)) if npairs is None else npairs
+    return md_pairs(_shells_struct(a), _shells_struct(b), int(n), _ptr(idx))
+
+
+class DeviceShells:
+    """A shell batch resident on the GPU (torch float64 tensors)."""
+
+    def __init__(self, l, K, center, exps, coefs):
+        self.l, self.K, self.center, self.exps, self.coefs = int(l), int(K), center, exps, coefs
+
+    @property
+    def n(self):
+        return self.center.shape[0]
+
+
+def to_device(shells, device="cuda"):
+    import torch
+    f = lambda a: torch.as_tensor(np.ascontiguousarray(a, dtype=np.float64)).to(device)
+    return DeviceShells(shells.l, shells.K, f(shells.center), f(shells.exps), f(shells.coefs))
+
+
+def idx_to_device(idx, device="cuda"):
+    import torch
+    if idx is None:
+        return None
+    return torch.as_tensor(np.ascontiguousarray(idx, dtype=np.int32)).to(device)
+
+
+def _stream_ptr(stream):
+    import torch
+    s = torch.cuda.current_stream() if stream is None else stream
+    return ctypes.c_void_p(s.cuda_stream)
+
+
+def ncomp(l, pure):
+    return 2 * l + 1 if pure else (l + 1) * (l + 2) // 2
+
+
+def md_init():
+    _check(lib().md_init())
+
+
+def md_set_variant(v):
+    _check(lib().md_set_variant(int(v)))
+
+
+def md_last_variant():
+    return lib().md_last_variant()
+
+
+def md_last_launch_count():
+    return lib().md_last_launch_count()
+
+
+def md_eri4_out_elems(la, lb, lc, ld, pure, n):
+    return lib().md_eri4_out_elems(la, lb, lc, ld, int(pure), n)
+
+
+def md_eri3_out_elems(la, lb, lX, pure, n):
+    return lib().md_eri3_out_elems(la, lb, lX, int(pure), n)
+
+
+def md_eri4(a, b, c, d, bra_idx, ket_idx, quartet_idx, nquartets, pure, out, layout=LAYOUT_QUARTET_MAJOR,
+            stream=None, nbra=None, nket=None):
+    """(ab|cd) on DEVICE tensors; `out` is a caller-owned torch float64 CUDA tensor.  Asynchronous."""
+    bra = _pairs_struct(a, b, bra_idx, nbra)
+    ket = _pairs_struct(c, d, ket_idx, nket)
+    _check(lib().md_eri4(ctypes.byref(bra), ctypes.byref(ket), int(nquartets), _ptr(quartet_idx), int(pure),
+                         int(layout), _ptr(out), out.numel(), _stream_ptr(stream)))
+    return out
+
+
+def md_eri3(a, b, x, bra_idx, triplet_idx, ntriplets, pure, out, layout=LAYOUT_QUARTET_MAJOR, stream=None,
+            nbra=None):
+    """(ab|X) on DEVICE tensors.  Asynchronous."""
+    bra = _pairs_struct(a, b, bra_idx, nbra)
+    xs = _shells_struct(x)
+    _check(lib().md_eri3(ctypes.byref(bra), ctypes.byref(xs), int(ntriplets), _ptr(triplet_idx), int(pure),
+                         int(layout), _ptr(out), out.numel(), _stream_ptr(stream)))
+    return out
+
+
+def md_eri4_host(a, b, c, d, bra_idx, ket_idx, quartet_idx, nquartets, pure, out, layout=LAYOUT_QUARTET_MAJOR,
+                 stream=None, nbra=None, nket=None):
+    """(ab|cd) on HOST arrays (numpy or pinned torch CPU tensors); copies are inside the call."""
+    bra = _pairs_struct(a, b, bra_idx, nbra)
+    ket = _pairs_struct(c, d, ket_idx, nket)
+    nout = out.size if isinstance(out, np.ndarray) else out.numel()
+    _check(lib().md_eri4_host(ctypes.byref(bra), ctypes.byref(ket), int(nquartets), _ptr(quartet_idx), int(pure),
+                              int(layout), _ptr(out), nout, _stream_ptr(stream)))
+    return out
+
+
+def md_eri3_host(a, b, x, bra_idx, triplet_idx, ntriplets, pure, out, layout=LAYOUT_QUARTET_MAJOR, stream=None,
+                 nbra=None):
+    bra = _pairs_struct(a, b, bra_idx, nbra)
+    xs = _shells_struct(x)
+    nout = out.size if isinstance(out, np.ndarray) else out.numel()
+    _check(lib().md_eri3_host(ctypes.byref(bra), ctypes.byref(xs), int(ntriplets), _ptr(triplet_idx), int(pure),
+                              int(layout), _ptr(out), nout, _stream_ptr(stream)))
+    return out
+
+
+def md_boys(mmax, T):
+    """F_m(T) for a torch CUDA float64 vector T -> [n, mmax+1] (the kernels' device routine)."""
+    import torch
+    out = torch.empty((T.numel(), mmax + 1), dtype=torch.float64, device=T.device)
+    _check(lib().md_boys(int(mmax), T.numel(), _ptr(T), _ptr(out), _stream_ptr(None)))
+    return out
+
+
+def md_fp64_peak(kind, seconds=0.5):
+    """Measured FP64 issue-loop rate in TFLOP/s: kind 0 DFMA, 1 DMMA m8n8k4, 2 DMMA m16n8k8."""
+    tf, ms = ctypes.c_double(0), ctypes.c_double(0)
+    _check(lib().md_fp64_peak(int(kind), max(1, int(seconds * 10)), ctypes.byref(tf), ctypes.byref(ms)))
+    return tf.value, ms.value
+
+
+class DeviceWorkload:
+    """A workloads.Workload with its arrays copied to the GPU once (inputs resident in HBM)."""
+
+    def __init__(self, w, device="cuda"):
+        self.w = w
+        self.a, self.b, self.c = to_device(w.a, device), to_device(w.b, device), to_device(w.c, device)
+        self.d = None if w.three_center else to_device(w.d, device)
+        self.bra_idx = idx_to_device(w.bra_idx, device)
+        self.ket_idx = idx_to_device(w.ket_idx, device)
+        self.quartet_idx = idx_to_device(w.quartet_idx, device)
+
+    def alloc_out(self, pure):
+        import torch
+        return torch.empty(self.w.nquartets * self.w.nout(pure), dtype=torch.float64, device=self.a.center.device)
+
+    def run(self, pure, out=None, layout=LAYOUT_QUARTET_MAJOR, stream=None):
+        w = self.w
+        out = self.alloc_out(pure) if out is None else out
+        if w.three_center:
+            return md_eri3(self.a, self.b, self.c, self.bra_idx, self.quartet_idx, w.nquartets, pure, out, layout,
+                           stream, nbra=w.nbra)
+        return md_eri4(self.a, self.b, self.c, self.d, self.bra_idx, self.ket_idx, self.quartet_idx, w.nquartets,
+                       pure, out, layout, stream, nbra=w.nbra, nket=w.nket)
+
+
+def run_host(w, pure, out, layout=LAYOUT_QUARTET_MAJOR, stream=None):
+    """The host-buffer call on a workloads.Workload (numpy arrays in, numpy/pinned array out)."""
+    if w.three_center:
+        return md_eri3_host(w.a, w.b, w.c, w.bra_idx, w.quartet_idx, w.nquartets, pure, out, layout, stream,
+                            nbra=w.nbra)
+    return md_eri4_host(w.a, w.b, w.c, w.d, w.bra_idx, w.ket_idx, w.quartet_idx, w.nquartets, pure, out, layout,
+                        stream, nbra=w.nbra, nket=w.nket)
