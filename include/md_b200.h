@@ -149,8 +149,10 @@ int md_last_launch_count(void);
 int md_init(void);
 
 /* Boys function F_m(T), m = 0..mmax <= 4*MD_MAX_L, for n values of T (device pointers;
- * out is [n][mmax+1]); the device routine the integral kernels use (Eq. 22). */
-int md_boys(int mmax, int64_t n, const double *T, double *out, void *cuda_stream);
+ * out is [n][mmax+1]): the device routines the integral kernels use (Eq. 22).
+ *   scheme 0: top order from the Taylor table + downward recursion (runtime-l kernel)
+ *   scheme 1: every order from the Taylor table independently (fused kernels) */
+int md_boys(int mmax, int scheme, int64_t n, const double *T, double *out, void *cuda_stream);
 
 /* Measurement helper (not on the hot path): best achieved FP64 rate, in TFLOP/s, of a pure
  * issue loop running for about seconds_x10/10 s on the current device.

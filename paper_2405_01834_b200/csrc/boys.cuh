@@ -9,13 +9,18 @@
 //   T >= MD_BOYS_TMAX : F_0 = (1/2) sqrt(pi/T) erf(sqrt T), then the upward recursion
 //                         F_{m+1} = ((2m+1) F_m - e^{-T}) / (2T).
 // |h| <= 1/32, so the first dropped Taylor term is below (1/32)^8/8! = 2.3e-17 of F_M.
-// The table (513 x 32 doubles, 128 KB) is built on the device at md_init() and stays in L2.
+// The fused kernels evaluate each order on its own thread (boys_single): the same Taylor
+// expansion for the wanted order m <= 24 (columns m..m+7 <= 31) for T < 128, and
+//   F_m(T) = (2m-1)!!/(2T)^m (1/2) sqrt(pi/T)       for T >= 128,
+// whose neglected part is below e^{-128} (reading S4) -- no exp, no recursion.
+// The table (2049 x 32 doubles, 512 KB) is built on the device at md_init() and stays in L2.
 #pragma once
 #include "common.cuh"
 
 #define MD_BOYS_MTAB 32
-#define MD_BOYS_NROW 513
-#define MD_BOYS_TMAX 32.0
+#define MD_BOYS_NROW 2049                 // T_i = i/16, 0 <= T_i <= 128
+#define MD_BOYS_TMAX 32.0                 // boys_eval: switch to erf + upward recursion
+#define MD_BOYS_TASY 127.96875            // boys_single: switch to the asymptotic form
 #define MD_BOYS_STEP 0.0625
 #define MD_BOYS_ISTEP 16.0
 
@@ -27,13 +32,13 @@ static __constant__ double c_inv_odd[MD_LTOT + 8];
 // Table row i: F_m(i/16), m = 0..31, by the ascending series at m = 31 (all terms positive),
 //   F_M(x) = e^{-x} sum_{k>=0} (2x)^k / [(2M+1)(2M+3)..(2M+2k+1)],
 // and the downward recursion.  One thread per row; runs once.
-__global__ void boys_table_kernel(double *tab) {
+static __global__ void boys_table_kernel(double *tab) {
     int i = blockIdx.x * blockDim.x + threadIdx.x;
     if (i >= MD_BOYS_NROW) return;
     const int M = MD_BOYS_MTAB - 1;
     double x = i * MD_BOYS_STEP;
     double term = 1.0 / (2 * M + 1), sum = term;
-    for (int k = 1; k < 1000; ++k) {
+    for (int k = 1; k < 4000; ++k) {
         term *= 2.0 * x / (2 * M + 2 * k + 1);
         sum += term;
         if (term < 1e-18 * sum) break;
@@ -80,7 +85,29 @@ __device__ __forceinline__ void boys_eval(int mmax, double T, const double *__re
     }
 }
 
-// Compile-time-order variant for the fused kernels: F lives in registers.
+// One order, independent of the others (fused kernels: one thread per (quartet, m)).
+__device__ __forceinline__ double boys_single(int m, double T, const double *__restrict__ tab) {
+    if (T < MD_BOYS_TASY) {
+        const int i = __double2int_rn(T * MD_BOYS_ISTEP);
+        const double mh = i * MD_BOYS_STEP - T;
+        const double *r = tab + i * MD_BOYS_MTAB + m;
+        double s = __ldg(r + 7) * (1.0 / 5040.0);
+        s = fma(s, mh, __ldg(r + 6) * (1.0 / 720.0));
+        s = fma(s, mh, __ldg(r + 5) * (1.0 / 120.0));
+        s = fma(s, mh, __ldg(r + 4) * (1.0 / 24.0));
+        s = fma(s, mh, __ldg(r + 3) * (1.0 / 6.0));
+        s = fma(s, mh, __ldg(r + 2) * 0.5);
+        s = fma(s, mh, __ldg(r + 1));
+        return fma(s, mh, __ldg(r));
+    }
+    const double it = 1.0 / T;
+    double f = 0.88622692545275801365 * sqrt(it);
+    const double h = 0.5 * it;
+    for (int k = 0; k < m; ++k) f *= (2 * k + 1) * h;
+    return f;
+}
+
+// Compile-time-order variant: F lives in registers.
 template <int M>
 __device__ __forceinline__ void boys_eval_t(double T, const double *__restrict__ tab, double (&F)[M + 1]) {
     double ex = exp(-T);
@@ -117,11 +144,12 @@ __device__ __forceinline__ void boys_eval_t(double T, const double *__restrict__
 }
 
 // Test entry (md_boys): out[n][mmax+1].
-__global__ void boys_batch_kernel(int mmax, long long n, const double *T, const double *tab, double *out) {
+static __global__ void boys_batch_kernel(int mmax, int scheme, long long n, const double *T, const double *tab, double *out) {
     long long i = blockIdx.x * (long long)blockDim.x + threadIdx.x;
     if (i >= n) return;
     double F[MD_LTOT + 1];
-    boys_eval(mmax, T[i], tab, F);
+    if (scheme == 0) boys_eval(mmax, T[i], tab, F);
+    else for (int m = 0; m <= mmax; ++m) F[m] = boys_single(m, T[i], tab);
     for (int m = 0; m <= mmax; ++m) out[i * (mmax + 1) + m] = F[m];
 }
 

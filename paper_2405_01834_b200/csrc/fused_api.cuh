@@ -1,0 +1,15 @@
+// fused_api.cuh -- what md_b200.cu sees of the fused kernels (they are compiled in fused_inst.cu).
+#pragma once
+#include "common.cuh"
+
+namespace mdb {
+
+cudaError_t fused_upload_tables(const uint32_t *herm, const double *solid);
+cudaError_t fused_register_all(int max_smem);
+static inline cudaError_t fused_init(int max_smem) { return fused_register_all(max_smem); }
+
+// Returns 1 if a fused kernel was launched, 0 if the class has none, < 0 on error.
+int fused_dispatch(const PairView &b, const PairView &k, long long nq, const int32_t *qidx, int pure, int layout,
+                   double *out, const double *boys_tab, int nsm, cudaStream_t st, bool force);
+
+}  // namespace mdb

@@ -10,7 +10,7 @@
 #include "../../include/md_b200.h"
 #include "boys.cuh"
 #include "common.cuh"
-#include "fused.cuh"
+#include "fused_api.cuh"
 #include "generic.cuh"
 #include "pair.cuh"
 #include "peak.cuh"
@@ -242,7 +242,7 @@ int md_init(void) {
     CK(cudaMemcpyToSymbol(c_inv_odd, inv, sizeof(inv)));
     if (S.boys_tab) cudaFree(S.boys_tab);
     CK(cudaMalloc(&S.boys_tab, sizeof(double) * MD_BOYS_NROW * MD_BOYS_MTAB));
-    boys_table_kernel<<<(MD_BOYS_NROW + 127) / 128, 128>>>(S.boys_tab);
+    boys_table_kernel<<<(MD_BOYS_NROW + 63) / 64, 64>>>(S.boys_tab);
     CK(cudaGetLastError());
     CK(cudaDeviceGetAttribute(&S.nsm, cudaDevAttrMultiProcessorCount, dev));
     CK(cudaDeviceGetAttribute(&S.max_smem, cudaDevAttrMaxSharedMemoryPerBlockOptin, dev));
@@ -307,12 +307,12 @@ int md_set_variant(int v) {
 int md_last_variant(void) { return S.last_variant; }
 int md_last_launch_count(void) { return S.last_launches; }
 
-int md_boys(int mmax, int64_t n, const double *T, double *out, void *cuda_stream) {
-    if (mmax < 0 || mmax > MD_LTOT || n < 0 || (n > 0 && (!T || !out))) return MD_EINVAL;
+int md_boys(int mmax, int scheme, int64_t n, const double *T, double *out, void *cuda_stream) {
+    if (mmax < 0 || mmax > MD_LTOT || n < 0 || (n > 0 && (!T || !out)) || scheme < 0 || scheme > 1) return MD_EINVAL;
     int e = md_init();
     if (e) return e;
     if (n == 0) return MD_OK;
-    boys_batch_kernel<<<(unsigned)((n + 127) / 128), 128, 0, (cudaStream_t)cuda_stream>>>(mmax, n, T, S.boys_tab, out);
+    boys_batch_kernel<<<(unsigned)((n + 127) / 128), 128, 0, (cudaStream_t)cuda_stream>>>(mmax, scheme, n, T, S.boys_tab, out);
     CK(cudaGetLastError());
     return MD_OK;
 }

@@ -60,7 +60,7 @@ def lib():
         L.md_eri3_workspace_bytes.restype = ctypes.c_int64
         L.md_set_workspace.argtypes = [ctypes.c_void_p, ctypes.c_size_t]
         L.md_set_variant.argtypes = [ctypes.c_int]
-        L.md_boys.argtypes = [ctypes.c_int, ctypes.c_int64, ctypes.c_void_p, ctypes.c_void_p, ctypes.c_void_p]
+        L.md_boys.argtypes = [ctypes.c_int, ctypes.c_int, ctypes.c_int64, ctypes.c_void_p, ctypes.c_void_p, ctypes.c_void_p]
         L.md_fp64_peak.argtypes = [ctypes.c_int, ctypes.c_int, _dp, _dp]
         L.md_strerror.argtypes = [ctypes.c_int]
         L.md_strerror.restype = ctypes.c_char_p
@@ -202,11 +202,11 @@ def md_eri3_host(a, b, x, bra_idx, triplet_idx, ntriplets, pure, out, layout=LAY
     return out
 
 
-def md_boys(mmax, T):
-    """F_m(T) for a torch CUDA float64 vector T -> [n, mmax+1] (the kernels' device routine)."""
+def md_boys(mmax, T, scheme=0):
+    """F_m(T) for a torch CUDA float64 vector T -> [n, mmax+1] (the kernels' device routines)."""
     import torch
     out = torch.empty((T.numel(), mmax + 1), dtype=torch.float64, device=T.device)
-    _check(lib().md_boys(int(mmax), T.numel(), _ptr(T), _ptr(out), _stream_ptr(None)))
+    _check(lib().md_boys(int(mmax), int(scheme), T.numel(), _ptr(T), _ptr(out), _stream_ptr(None)))
     return out
 
 

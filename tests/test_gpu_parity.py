@@ -26,16 +26,18 @@ def test_boys_device_vs_mpmath():
     import mpmath as mp
     import torch
     mp.mp.dps = 40
-    T = np.concatenate([[0.0, 1e-12, 1e-6, 0.03124, 0.03126, 0.09375, 31.96, 31.9999999, 32.0, 32.0000001, 40.0, 1e3, 3e4],
-                        np.random.default_rng(1).uniform(0, 60, 500), np.exp(np.random.default_rng(2).uniform(-20, 11, 300))])
+    T = np.concatenate([[0.0, 1e-12, 1e-6, 0.03124, 0.03126, 0.09375, 31.96, 31.9999999, 32.0, 32.0000001, 40.0, 127.9,
+                         127.96874, 127.96875, 127.97, 128.0, 131.0, 1e3, 3e4],
+                        np.random.default_rng(1).uniform(0, 140, 600), np.exp(np.random.default_rng(2).uniform(-20, 11, 300))])
     worst = 0.0
-    for mmax in (0, 1, 8, 24):
-        F = engine.md_boys(mmax, torch.as_tensor(T).cuda()).cpu().numpy()
-        for m in sorted({0, mmax // 2, mmax}):
-            ref = np.array([float(mp.hyp1f1(m + 0.5, m + 1.5, -mp.mpf(float(t))) / (2 * m + 1)) for t in T])
-            rel = np.abs(F[:, m] - ref) / ref
-            worst = max(worst, rel.max())
-            assert rel.max() < 2e-14, (mmax, m, rel.max(), T[rel.argmax()])
+    for scheme in (0, 1):
+        for mmax in (0, 1, 8, 24):
+            F = engine.md_boys(mmax, torch.as_tensor(T).cuda(), scheme).cpu().numpy()
+            for m in sorted({0, mmax // 2, mmax}):
+                ref = np.array([float(mp.hyp1f1(m + 0.5, m + 1.5, -mp.mpf(float(t))) / (2 * m + 1)) for t in T])
+                rel = np.abs(F[:, m] - ref) / ref
+                worst = max(worst, rel.max())
+                assert rel.max() < 2e-14, (scheme, mmax, m, rel.max(), T[rel.argmax()])
     print("boys worst rel", worst)
 
 
