@@ -133,13 +133,14 @@ int md_set_workspace(void *device_ptr, size_t bytes);
 
 /* Kernel-variant control, for measurement:
  *   MD_VARIANT_AUTO    the measured-best variant per class (default)
- *   MD_VARIANT_GENERIC the runtime-l kernel chain (pair setup + quartet kernel) for every class
+ *   MD_VARIANT_GENERIC the runtime-l kernel chain (pair setup + DFMA quartet kernel) for every class
  *   MD_VARIANT_FUSED   the compile-time-l fused kernel where one exists, else generic  */
 #define MD_VARIANT_AUTO    0
 #define MD_VARIANT_GENERIC 1
 #define MD_VARIANT_FUSED   2
+#define MD_VARIANT_MMA     3     /* pair setup + the DMMA (mma.sync f64) quartet kernel for every class */
 int md_set_variant(int variant);
-/* Which variant the last md_eri4/md_eri3 call used (MD_VARIANT_GENERIC or MD_VARIANT_FUSED),
+/* Which variant the last md_eri4/md_eri3 call used (MD_VARIANT_GENERIC, _FUSED or _MMA),
  * and how many kernels it launched. */
 int md_last_variant(void);
 int md_last_launch_count(void);

@@ -6,6 +6,7 @@ namespace mdb {
 
 cudaError_t fused_upload_tables(const uint32_t *herm, const double *solid);
 cudaError_t fused_register_all(int max_smem);
+const uint32_t *fused_rlut();   // [2*N~(24)] R-recursion LUT (device), shared with the DMMA kernels
 static inline cudaError_t fused_init(int max_smem) { return fused_register_all(max_smem); }
 
 // Returns 1 if a fused kernel was launched, 0 if the class has none, < 0 on error.

@@ -15,7 +15,7 @@ cudaError_t fused_upload_tables(const uint32_t *herm, const double *solid) {
     // R-recursion LUT (Eq. 24): for Hermite entry e = (t,u,v) of the degree-sorted list,
     // word 0 = i1 | i2 << 12 | axis << 24 | coef << 26 with
     //   [e]^(m) = PQ[axis] * [i1]^(m+1) + coef * [i2]^(m+1),  i1 = e - 1_axis, i2 = e - 2_axis, coef = e_axis - 1
-    // on the first axis with a non-zero index; word 1 = packed (t,u,v).
+    // on the first axis with a non-zero index; word 1 = packed (t,u,v,n).
     std::vector<uint32_t> lut(2 * MD_NHERM_MAX);
     for (int k = 0; k < MD_NHERM_MAX; ++k) {
         int t = herm[k] & 0xff, u = herm[k] >> 8 & 0xff, v = herm[k] >> 16 & 0xff;
@@ -24,7 +24,7 @@ cudaError_t fused_upload_tables(const uint32_t *herm, const double *solid) {
         else if (u > 0) w = herm_index(t, u - 1, v) | (u > 1 ? herm_index(t, u - 2, v) : 0) << 12 | 1u << 24 | (uint32_t)(u - 1) << 26;
         else if (v > 0) w = herm_index(t, u, v - 1) | (v > 1 ? herm_index(t, u, v - 2) : 0) << 12 | 2u << 24 | (uint32_t)(v - 1) << 26;
         lut[2 * k] = w;
-        lut[2 * k + 1] = herm[k] & 0xffffff;
+        lut[2 * k + 1] = herm[k];               // t | u<<8 | v<<16 | n<<24
     }
     if (!g_rlut) {
         e = cudaMalloc(&g_rlut, lut.size() * sizeof(uint32_t));

@@ -12,6 +12,7 @@
 #include "common.cuh"
 #include "fused_api.cuh"
 #include "generic.cuh"
+#include "mma_api.cuh"
 #include "pair.cuh"
 #include "peak.cuh"
 
@@ -30,6 +31,7 @@ struct State {
     int variant = MD_VARIANT_AUTO;
     int last_variant = 0;
     int last_launches = 0;
+    int last_mma_info[8] = {0};
     int nsm = 148;
     int max_smem = 227 * 1024;
     char cuda_err[256] = "";
@@ -163,7 +165,7 @@ void out_strides(int layout, bool list_mode, long long nbra, long long nket, int
 }
 
 int run_generic(const PairView &b, const PairView &k, long long nq, const int32_t *qidx, int pure, int layout,
-                double *out, cudaStream_t st) {
+                double *out, cudaStream_t st, bool use_mma) {
     Shape s = shape_of(b, k, pure);
     void *ws = nullptr;
     int e = get_workspace(generic_ws_bytes(b, k, pure), &ws);
@@ -188,6 +190,20 @@ int run_generic(const PairView &b, const PairView &k, long long nq, const int32_
     ct = std::min<long long>(ct, std::max(16, 4096 / s.nhb));
     g.ct = (int)std::min<long long>(ct, s.ncd);
     size_t smem = fixed + 8 * (size_t)s.nhb * g.ct;
+    if (use_mma) {
+        MmaCall c;
+        c.rec_bra = rec_b; c.rec_ket = rec_k; c.stride_bra = s.stride_b; c.stride_ket = s.stride_k;
+        c.Kbra = g.Kbra; c.Kket = g.Kket; c.Lb = g.Lb; c.Lk = g.Lk; c.nab = s.nab; c.ncd = s.ncd;
+        // one-centre solid ket (Hobson, pair.cuh): Hermite rows of order < l_X are exactly zero
+        c.kq0 = (k.single && pure) ? nherm(k.a.l - 1) : 0;
+        c.qidx = qidx; c.nq = nq; c.nket = k.npairs; c.out = out;
+        c.s_q = g.s_q; c.s_bi = g.s_bi; c.s_ki = g.s_ki; c.s_ab = g.s_ab; c.s_cd = g.s_cd;
+        c.boys_tab = S.boys_tab; c.rlut = fused_rlut();
+        CK(mma_launch(c, S.nsm, st, S.last_mma_info));
+        S.last_launches++;
+        S.last_variant = MD_VARIANT_MMA;
+        return MD_OK;
+    }
     unsigned grid = (unsigned)std::min<long long>(nq, (long long)S.nsm * 8);
     eri_generic_kernel<<<grid, MD_GEN_THREADS, smem, st>>>(g);
     S.last_launches++;
@@ -210,7 +226,7 @@ int run(const PairView &b, const PairView &k, long long nq, const int32_t *qidx,
     if (e) return e;
     S.last_launches = 0;
     if (nq == 0) return MD_OK;
-    if (S.variant != MD_VARIANT_GENERIC) {
+    if (S.variant == MD_VARIANT_AUTO || S.variant == MD_VARIANT_FUSED) {
         int r = fused_dispatch(b, k, nq, qidx, pure, layout, out, S.boys_tab, S.nsm, st, S.variant == MD_VARIANT_FUSED);
         if (r == 1) {
             S.last_launches++;
@@ -220,7 +236,7 @@ int run(const PairView &b, const PairView &k, long long nq, const int32_t *qidx,
         }
         if (r < 0) return r;
     }
-    return run_generic(b, k, nq, qidx, pure, layout, out, st);
+    return run_generic(b, k, nq, qidx, pure, layout, out, st, S.variant != MD_VARIANT_GENERIC);
 }
 
 }  // namespace
@@ -249,6 +265,7 @@ int md_init(void) {
     CK(cudaFuncSetAttribute(eri_generic_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, S.max_smem - 1024));
     CK(cudaFuncSetAttribute(pair_setup_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, 96 * 1024));
     CK(fused_init(S.max_smem));
+    CK(mma_init(S.max_smem));
     CK(cudaDeviceSynchronize());
     S.init = true;
     S.device = dev;
@@ -300,7 +317,7 @@ int md_set_workspace(void *p, size_t bytes) {
     return MD_OK;
 }
 int md_set_variant(int v) {
-    if (v < MD_VARIANT_AUTO || v > MD_VARIANT_FUSED) return MD_EINVAL;
+    if (v < MD_VARIANT_AUTO || v > MD_VARIANT_MMA) return MD_EINVAL;
     S.variant = v;
     return MD_OK;
 }

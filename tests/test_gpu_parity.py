@@ -12,6 +12,7 @@ from gpu_util import assert_parity, check, gpu_run, oracle_run
 pytestmark = pytest.mark.gpu
 
 GENERIC = engine.VARIANT_GENERIC
+MMA = engine.VARIANT_MMA
 
 
 def _n_for(ls):
@@ -79,10 +80,22 @@ def test_class_auto_vs_oracle(ls):
         check(W.clustered(ls, max(3, n // 4)), pure)
 
 
+@pytest.mark.parametrize("ls", CLASSES, ids=lambda ls: "".join(map(str, ls)))
+def test_class_mma_vs_oracle(ls):
+    """The DMMA quartet kernel on every class, including those AUTO serves with a fused kernel."""
+    n = _n_for(ls)
+    for pure in (True, False):
+        if not pure and sum(ls) > 16:
+            continue
+        _, used = check(W.class_sweep(ls, n), pure, MMA)
+        assert used == MMA
+        check(W.clustered(ls, max(3, n // 4)), pure, MMA)
+
+
 @pytest.mark.parametrize("coincide", ["AB", "CD", "ALL"])
 @pytest.mark.parametrize("ls", [(1, 1, 1, 1), (2, 2, 2, 2), (3, 2, 1, 0), (4, 4, 2, 2)], ids=lambda ls: "".join(map(str, ls)))
 def test_degenerate_geometry(ls, coincide):
-    for variant in (engine.VARIANT_AUTO, GENERIC):
+    for variant in (engine.VARIANT_AUTO, GENERIC, MMA):
         check(W.clustered(ls, 23, coincide=coincide), True, variant)
         check(W.clustered(ls, 23, coincide=coincide), False, variant)
 
@@ -93,7 +106,7 @@ def test_degenerate_geometry(ls, coincide):
                                    ((2, 2, 2, 2), (3, 3, 3, 3)), ((2, 1, 0, 2), (2, 1, 4, 3)), ((3, 3, 2, 2), (2, 2, 1, 3)),
                                    ((4, 2, 3, 1), (1, 2, 2, 1))])
 def test_contracted_classes(ls, Ks):
-    for variant in (engine.VARIANT_AUTO, GENERIC):
+    for variant in (engine.VARIANT_AUTO, GENERIC, MMA):
         w = W.independent_quartets("contr", ls, Ks, 67, (0.05, 50.0), (-2.0, 2.0), W.class_seed("contr", ls, Ks))
         check(w, True, variant)
         check(w, False, variant)
@@ -113,7 +126,7 @@ def test_config2_dddd_K1_and_K3_sampled():
                                       (0, 3, 5), (4, 4, 4), (6, 6, 6), (0, 0, 6), (6, 5, 0)])
 def test_three_center(la, lb, lX):
     n = _n_for((la, lb, lX))
-    for variant in (engine.VARIANT_AUTO, GENERIC):
+    for variant in (engine.VARIANT_AUTO, GENERIC, MMA):
         for pure in (True, False):
             check(W.class_sweep((la, lb, lX), n, K=(1, 1, 1), three_center=True), pure, variant)
             check(W.clustered((la, lb, lX), max(3, n // 4), K=(1, 1, 1), three_center=True), pure, variant)
@@ -135,7 +148,7 @@ def _product(ls, nbra, nket, three_center=False, K=1):
 @pytest.mark.parametrize("ls", [(1, 1, 1, 1), (2, 1, 2, 0), (2, 2, 2, 2), (3, 3, 1, 1)], ids=lambda ls: "".join(map(str, ls)))
 def test_product_mode_and_paper_layout(ls):
     w = _product(ls, 13, 7)
-    for variant in (engine.VARIANT_AUTO, GENERIC):
+    for variant in (engine.VARIANT_AUTO, GENERIC, MMA):
         for pure in (True, False):
             ref = oracle_run(w, pure)                                        # [nbra*nket, nout], ket fastest
             gpu, _ = gpu_run(w, pure, variant)
@@ -158,7 +171,7 @@ def test_pair_index_lists_and_shared_shells():
     ket_idx = np.stack([rng.integers(0, 5, 17), rng.integers(0, 6, 17)], 1).astype(np.int32)
     qi = np.stack([rng.integers(0, 31, 211), rng.integers(0, 17, 211)], 1).astype(np.int32)
     w = W.Workload("idx", a, b, c, d, bra_idx, ket_idx, qi)
-    for variant in (engine.VARIANT_AUTO, GENERIC):
+    for variant in (engine.VARIANT_AUTO, GENERIC, MMA):
         check(w, True, variant)
         check(w, False, variant)
     w2 = W.Workload("idxprod", a, b, c, d, bra_idx, ket_idx, None)
