@@ -147,7 +147,7 @@ def measure_variant(dw, w, K, pure, steps, warmup, flush, barrier):
     flops = W.flops_model(2, 2, 2, 2, K * K, K * K, pure)
     return {"K": K, "pure": pure, "ms_per_step": ms / steps, "quartets_per_s": w.nquartets * steps / (ms * 1e-3),
             "model_flop_per_quartet": flops, "model_tflops": flops * w.nquartets * steps / (ms * 1e-3) / 1e12,
-            "variant": {1: "generic", 2: "fused"}.get(engine.md_last_variant(), "?"),
+            "variant": {1: "generic", 2: "fused", 3: "mma", 4: "fused2"}.get(engine.md_last_variant(), "?"),
             "launches_per_step": engine.md_last_launch_count(), "out_bytes": out.numel() * 8}
 
 

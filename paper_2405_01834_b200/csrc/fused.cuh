@@ -21,6 +21,8 @@ struct FusedEntry {
 
 // [la][lb][lc][ld][pure]; only canonical entries are filled.
 FusedEntry *fused_table();
+void fused_make_args(const PairView &b0, const PairView &k0, long long nq, const int32_t *qidx, int pure, int layout,
+                     double *out, const double *boys_tab, FusedArgs &g, int l[4]);
 cudaError_t fused_register_all(int max_smem);   // defined in fused_inst.cu
 
 template <int LA, int LB, int LC, int LD, bool PURE>

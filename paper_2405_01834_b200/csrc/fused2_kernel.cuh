@@ -1,0 +1,207 @@
+// fused2_kernel.cuh -- warp-specialised compile-time-l fused kernel: ONE launch runs S1-S5 of a class
+// (la lb|lc ld) with no intermediate in HBM, built for contracted shells.
+//
+// A CTA holds NC consumer threads and NP producer threads and works on NQ quartets at a time.
+// For every bra primitive kb and ket primitive kk (a "batch" = that primitive quartet of all NQ
+// quartets) the PRODUCER warps build, in one of two shared-memory buffers,
+//   stage 0  the ket 1-D tables E^t_{ij} of primitive kk               (Eqs. 9,10,13,14)
+//   stage 1  [0]^(m) (Eqs. 21-23, Boys function) and from it the z-line [00v]^(m);
+//            the ket products E^{cd}_{q~}(-1)^{|q~|}, q~-major               (Eqs. 7, 19)
+//   stage y  [0uv]^(m) from [00v]^(m)                                         (Eq. 24 on u)
+//   stage x  [tuv]^(0) from [0uv]^(m), stored in an additive bank-aware layout   (Eq. 24 on t)
+// while the CONSUMER warps contract the other buffer,
+//   P4  [p~|cd] += sum_q~ E^{cd}_{q~} [p~+q~]^(0)                              (Eq. 25)
+// each thread owning PB Hermite rows p~ and one chunk of cd in REGISTERS for the whole kk loop.
+// Eq. 24 is applied one Cartesian direction at a time: a thread that owns a line (all t for fixed
+// u,v) needs only the [0uv]^(m), m = 0..L-u-v, of that line and two register rows, so the
+// recursion costs three producer-only barriers per batch instead of one CTA barrier per level.
+// The two buffers are handed over with named barriers (bar.arrive / bar.sync).
+// After the kk loop of a bra primitive the whole CTA transforms the ket to solid harmonics
+// (Eq. 16), applies Eq. 26 ([ab|cd] += sum_p~ E^{ab}_{p~} [p~|cd]) with the bra transform, and
+// accumulates into the output block, which stays in L2 between bra primitives.
+#pragma once
+#include "boys.cuh"
+#include "fused2_tables.cuh"
+#include "fused_kernel.cuh"      // axis_table, solid2, FusedArgs
+
+namespace mdb {
+
+#define MD_F2_PRODUCERS 192          // two groups of three warps
+
+template <int LA, int LB, int LC, int LD, bool PURE, int PB, int NCH>
+struct F2Cfg {
+    static constexpr int Lb = LA + LB, Lk = LC + LD, L = Lb + Lk;
+    static constexpr int NHB = nherm(Lb), NHK = nherm(Lk), NHL = nherm(L);
+    static constexpr int NCA = ncart(LA), NCB = ncart(LB), NCC = ncart(LC), NCD = ncart(LD);
+    static constexpr int NAO = ncomp(LA, PURE), NBO = ncomp(LB, PURE), NCO = ncomp(LC, PURE), NDO = ncomp(LD, PURE);
+    static constexpr int NAB_C = NCA * NCB, NAB_O = NAO * NBO, NCD_O = NCO * NDO;
+    static constexpr int NPG = (NHB + PB - 1) / PB;            // p~ groups per quartet
+    static constexpr int CHC = (NCC + NCH - 1) / NCH;          // c components per chunk
+    static constexpr int NACC = CHC * NCD;                     // accumulators per p~
+    static constexpr int E1B = e1_count(LA, LB), E1K = e1_count(LC, LD);
+    static constexpr int TB = even_up(8 + 3 * E1B), TK = even_up(8 + 3 * E1K);   // table records
+    static constexpr int NPB = ProdCount<LA, LB>::value();
+    static constexpr int EPK = ProdQ<LC, LD, NCH>{}.len();
+    static constexpr int HW = NCC * NDO;                       // [c][md] before the c transform
+    static constexpr int HS = HW | 1;                          // odd row stride: conflict-free columns
+    static constexpr int NZ = (L + 1) * (L + 2) / 2;           // entries of the z-line output
+    // one batch record per quartet (doubles)
+    static constexpr Brick BR = brick_layout(L, Lb);
+    static_assert(brick_injective(L, BR), "brick layout must be injective");
+    static constexpr int NRA = even_up(BR.foot > NZ ? BR.foot : NZ);
+    static constexpr int O_A = 0;                              // z-line output, later [r]^(0) in the brick layout
+    static constexpr int O_B = O_A + NRA;                      // [0uv]^(m) columns
+    static constexpr int O_PQ = O_B + even_up(NHL);            // X, Y, Z, pad
+    static constexpr int O_TK = O_PQ + 4;                      // ket table record
+    static constexpr int O_EP = O_TK + TK;                     // ket product list
+    static constexpr int BREC = O_EP + even_up(EPK);
+    // per quartet, outside the batch buffers
+    static constexpr int PERQ = 2 /*sidx*/ + 2 /*out base, flags*/ + TB + even_up(NPB) + NHB * HS + (NHB * HS & 1);
+    static constexpr int FIXED = (even_up(EPK) + even_up(NPB)) / 2;    // packed product words (doubles)
+    static __host__ __device__ constexpr size_t smem_bytes(int nq) { return 8 * ((size_t)nq * (PERQ + 2 * BREC) + FIXED); }
+};
+
+__device__ __forceinline__ void bar_sync(int id, int n) { asm volatile("bar.sync %0, %1;" ::"r"(id), "r"(n) : "memory"); }
+__device__ __forceinline__ void bar_arrive(int id, int n) {
+    __threadfence_block();
+    asm volatile("bar.arrive %0, %1;" ::"r"(id), "r"(n) : "memory");
+}
+enum { F2_BAR_PALL = 1, F2_BAR_FULL = 2, F2_BAR_EMPTY = 4, F2_BAR_PROD = 6 };
+
+// One axis of the two-centre table, written compactly (rows (i,j), t = 0..i+j).
+template <int L1, int L2>
+__device__ __forceinline__ void axis_table_compact(double za, double zb, double xab, double *E) {
+    constexpr int NT = L1 + L2 + 1;
+    double tmp[(L1 + 1) * (L2 + 1) * NT];
+    axis_table<L1, L2>(za, zb, xab, tmp);
+#pragma unroll
+    for (int i = 0; i <= L1; ++i)
+#pragma unroll
+        for (int j = 0; j <= L2; ++j)
+#pragma unroll
+            for (int t = 0; t <= i + j; ++t) E[e1_rowoff(L2, i, j) + t] = tmp[(i * (L2 + 1) + j) * NT + t];
+}
+
+// Table record of one primitive pair: rec[0] = p, rec[1..3] = P, rec[4] = c_a c_b, rec[8 + ax*E1 + ..].
+template <int L1, int L2>
+__device__ __forceinline__ void table_task(const PairView &pv, long long i1, long long i2, int k1, int k2, int ax, double *rec) {
+    constexpr int E1 = e1_count(L1, L2);
+    const int K1 = pv.a.K, K2 = pv.b.K;
+    const double za = __ldg(pv.a.exps + i1 * K1 + k1), A = __ldg(pv.a.center + 3 * i1 + ax);
+    double zb = 0.0, B = A;
+    if (!pv.single) { zb = __ldg(pv.b.exps + i2 * K2 + k2); B = __ldg(pv.b.center + 3 * i2 + ax); }
+    axis_table_compact<L1, L2>(za, zb, A - B, rec + 8 + ax * E1);
+    const double p = za + zb;
+    rec[1 + ax] = (za * A + zb * B) / p;
+    if (ax == 0) {
+        rec[0] = p;
+        rec[4] = __ldg(pv.a.coefs + i1 * K1 + k1) * (pv.single ? 1.0 : __ldg(pv.b.coefs + i2 * K2 + k2));
+    }
+}
+
+// Eq. 24 along one direction.  a[0][m] = [..0..]^(m), m = 0..n, on entry; after step t the row
+// a[(t+1)&1][m] holds [..t+1..]^(m), m = 0..n-t-1.  emit(t, row) is called for t = 0..n.
+template <int N, class Emit>
+__device__ __forceinline__ void line_recursion(double X, double (&a)[2][N + 1], int n, Emit &&emit) {
+    emit(std::integral_constant<int, 0>{}, a[0]);
+    static_for<N>([&](auto tc) {
+        constexpr int t = decltype(tc)::value;
+        if (t < n) {
+            double(&cur)[N + 1] = a[t & 1];
+            double(&nxt)[N + 1] = a[(t + 1) & 1];
+#pragma unroll
+            for (int m = 0; m < N - t; ++m) {
+                double v = X * cur[m + 1];
+                if (t > 0) v = fma((double)t, nxt[m + 1], v);
+                nxt[m] = v;
+            }
+            emit(std::integral_constant<int, t + 1>{}, nxt);
+        }
+    });
+}
+
+template <int LA, int LB, int LC, int LD, bool PURE, int PB, int NCH>
+struct F2Impl {
+    using C = F2Cfg<LA, LB, LC, LD, PURE, PB, NCH>;
+    static constexpr int L = C::L;
+
+    // ---- producer stages -------------------------------------------------------------------
+    // stage 1a: Boys function, [0]^(m) and the z-line for one tensor
+    static __device__ __forceinline__ void z_task(const double *bt, double *rec, const double *boys_tab) {
+        const double *kt = rec + C::O_TK;
+        const double p = bt[0], q = kt[0];
+        const double X = bt[1] - kt[1], Y = bt[2] - kt[2], Z = bt[3] - kt[3];
+        const double rho = p * q / (p + q);
+        double F[L + 1];
+        boys_eval_t<L>(rho * (X * X + Y * Y + Z * Z), boys_tab, F);
+        double a[2][L + 1];
+        double f = 34.98683665524972497 / (p * q * sqrt(p + q));          // 2 pi^{5/2}   (Eq. 21)
+        const double m2r = -2.0 * rho;
+#pragma unroll
+        for (int m = 0; m <= L; ++m) { a[0][m] = F[m] * f; f *= m2r; a[1][m] = 0.0; }
+        rec[C::O_PQ] = X; rec[C::O_PQ + 1] = Y; rec[C::O_PQ + 2] = Z;
+        double *zo = rec + C::O_A;
+        line_recursion<L>(Z, a, L, [&](auto vc, double(&row)[L + 1]) {
+            constexpr int v = decltype(vc)::value;
+            constexpr int off = v * (L + 1) - v * (v - 1) / 2;
+#pragma unroll
+            for (int m = 0; m <= L - v; ++m) zo[off + m] = row[m];
+        });
+    }
+    // stage y: thread owns v; [0uv]^(m) for u = 0..L-v, written as columns (u,v) of L-u-v+1 entries
+    static __device__ __forceinline__ void y_task(int v, double *rec) {
+        const int n = L - v;
+        const double *zo = rec + C::O_A + v * (L + 1) - v * (v - 1) / 2;
+        double a[2][L + 1];
+#pragma unroll
+        for (int m = 0; m <= L; ++m) { a[0][m] = m <= n ? zo[m] : 0.0; a[1][m] = 0.0; }
+        double *col = rec + C::O_B + (nherm(L) - nherm(n));                // block of this v
+        line_recursion<L>(rec[C::O_PQ + 1], a, n, [&](auto uc, double(&row)[L + 1]) {
+            constexpr int u = decltype(uc)::value;
+#pragma unroll
+            for (int m = 0; m <= L - u; ++m)
+                if (m <= n - u) col[m] = row[m];
+            col += n - u + 1;
+        });
+    }
+    // stage x: thread owns the line (u,v); emits [tuv]^(0) into the brick layout (fused2_tables.cuh)
+    static __device__ __forceinline__ void x_task(int u, int v, double *rec) {
+        const int nv = L - v, n = nv - u;
+        const double *col = rec + C::O_B + (nherm(L) - nherm(nv)) + u * (nv + 1) - u * (u - 1) / 2;
+        double a[2][L + 1];
+#pragma unroll
+        for (int m = 0; m <= L; ++m) { a[0][m] = m <= n ? col[m] : 0.0; a[1][m] = 0.0; }
+        double *R = rec + C::O_A + C::BR.B * u + v;
+        line_recursion<L>(rec[C::O_PQ], a, n, [&](auto tc, double(&row)[L + 1]) {
+            constexpr int t = decltype(tc)::value;
+            R[C::BR.A * t] = row[0];
+        });
+    }
+    // products of one Cartesian component pair, written at the positions POS gives
+    template <int L1, int L2, bool SIGN, class POS>
+    static __device__ __forceinline__ void prod_task(const double *tab, int comp, double *dst, POS &&pos) {
+        constexpr int NC2 = ncart(L2), E1 = e1_count(L1, L2);
+        const int c = comp / NC2, d = comp - c * NC2;
+        const int ea = d_cart<L1>.e[c], eb = d_cart<L2>.e[d];
+        const int ax = ea & 0xff, ay = ea >> 8 & 0xff, az = ea >> 16, bx = eb & 0xff, by = eb >> 8 & 0xff, bz = eb >> 16;
+        const short *ro = d_e1row<L1, L2>.off;
+        const double *Ex = tab + 8 + ro[ax * (L2 + 1) + bx];
+        const double *Ey = tab + 8 + E1 + ro[ay * (L2 + 1) + by];
+        const double *Ez = tab + 8 + 2 * E1 + ro[az * (L2 + 1) + bz];
+        const double coef = tab[4];
+        int i = 0;
+        for (int t = 0; t <= ax + bx; ++t) {
+            const double et = coef * Ex[t];
+            for (int u = 0; u <= ay + by; ++u) {
+                const double eu = et * Ey[u];
+                for (int v = 0; v <= az + bz; ++v, ++i) {
+                    double val = eu * Ez[v];
+                    if (SIGN && ((t + u + v) & 1)) val = -val;
+                    dst[pos(comp, i)] = val;
+                }
+            }
+        }
+    }
+};
+
+}  // namespace mdb

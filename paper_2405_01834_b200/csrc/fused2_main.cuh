@@ -1,0 +1,287 @@
+// fused2_main.cuh -- the kernel body of the warp-specialised fused kernel (see fused2_kernel.cuh).
+#pragma once
+#include "fused2_kernel.cuh"
+
+namespace mdb {
+
+struct Fused2Args {
+    FusedArgs f;                  // shells, index lists, output strides (as for fused_kernel)
+    int NQ;                       // quartets per CTA pass
+    int TCH;                      // consumer threads per cd chunk (multiple of 32, >= NQ*NPG)
+};
+
+// P4 for one batch and one cd chunk CH: hacc[k][comp] += E[e] * R[p_k + q(e)]   (Eq. 25).
+// Software-pipelined by hand: the E pairs are loaded ED pairs ahead and the Hermite integrals of a q~
+// group RD groups ahead of their use, into register rings indexed by compile-time constants, so that
+// the ~30-cycle shared-memory latency is covered inside one warp (there are only 1-2 consumer warps per
+// scheduler).
+template <class C, int LC, int LD, int PB, int NCH, int CH>
+__device__ __forceinline__ void f2_contract(double (&hacc)[PB][C::NACC], const double *Rb, const int (&pofs)[PB],
+                                            const double *EP) {
+    using QGT = QGroups<LC, LD, NCH, CH>;
+    constexpr ProdQ<LC, LD, NCH> PQ{};
+    constexpr int E0 = PQ.choff[CH], NE = PQ.choff[CH + 1] - E0, NPAIR = NE / 2;
+    constexpr int NG = QGT{}.ng;
+    constexpr int ED = 4, RD = 2;
+    const double2 *ep2 = (const double2 *)(EP + E0);
+    double2 eb[ED + 1];
+    double rb[RD + 1][PB];
+    auto loadR = [&](auto sc) {
+        constexpr int s = decltype(sc)::value;
+        constexpr XYZ h = herm_exp(QGT{}.gq[s]);
+        constexpr int qo = C::BR.A * h.x + C::BR.B * h.y + h.z;          // index(p~+q~) = index(p~) + index(q~)
+#pragma unroll
+        for (int k = 0; k < PB; ++k) rb[s % (RD + 1)][k] = Rb[pofs[k] + qo];
+    };
+    static_for<(RD < NG ? RD : NG)>([&](auto sc) { loadR(sc); });
+    static_for<(ED < NPAIR ? ED : NPAIR)>([&](auto pc) { eb[decltype(pc)::value % (ED + 1)] = ep2[decltype(pc)::value]; });
+    static_for<NE>([&](auto ec) {
+        constexpr int e = decltype(ec)::value;
+        constexpr int s = QGT{}.gid[e];
+        if constexpr ((e & 1) == 0 && e / 2 + ED < NPAIR) eb[(e / 2 + ED) % (ED + 1)] = ep2[e / 2 + ED];
+        if constexpr (s >= 0) {
+            constexpr bool starts = QGT{}.gs[s] == e && s + RD < NG;
+            if constexpr (starts) loadR(std::integral_constant<int, s + RD>{});
+            constexpr int comp = PQ.comp_of[E0 + e];
+            const double2 &p2 = eb[(e / 2) % (ED + 1)];
+            const double x = (e & 1) ? p2.y : p2.x;
+#pragma unroll
+            for (int k = 0; k < PB; ++k) hacc[k][comp] = fma(x, rb[s % (RD + 1)][k], hacc[k][comp]);
+        }
+    });
+}
+
+// One product-list entry from a table record and its packed word (fused2_tables.cuh).
+__device__ __forceinline__ double prod_entry(const double *tab, unsigned w) {
+    double v = tab[4] * tab[w & 1023] * (tab[w >> 10 & 1023] * tab[w >> 20 & 1023]);
+    if (w >> 30 & 1) v = -v;
+    return (w >> 31) ? v : 0.0;
+}
+
+// Flush of one chunk: ket d-index transform in registers (Eq. 16), rows to shared memory.
+template <class C, int LD, bool PURE, int PB>
+__device__ __forceinline__ void f2_flush(const double (&hacc)[PB][C::NACC], int c0, const int (&ip)[PB], double *half) {
+#pragma unroll
+    for (int k = 0; k < PB; ++k) {
+        if (ip[k] < 0) continue;
+        double *row = half + ip[k] * C::HS;
+#pragma unroll
+        for (int cl = 0; cl < C::CHC; ++cl) {
+            const int c = c0 + cl;
+            if (c >= C::NCC) break;
+            if constexpr (!PURE) {
+#pragma unroll
+                for (int d = 0; d < C::NCD; ++d) row[c * C::NCD + d] = hacc[k][cl * C::NCD + d];
+            } else {
+                constexpr SolidTab<LD> S{};
+#pragma unroll
+                for (int m = 0; m < C::NDO; ++m) {
+                    double s = 0.0;
+#pragma unroll
+                    for (int d = 0; d < C::NCD; ++d)
+                        if (S.c[m][d] != 0.0) s = fma(S.c[m][d], hacc[k][cl * C::NCD + d], s);
+                    row[c * C::NDO + m] = s;
+                }
+            }
+        }
+    }
+}
+
+template <int LA, int LB, int LC, int LD, bool PURE, int PB, int NCH>
+__global__ void __launch_bounds__(MD_F2_PRODUCERS + 192, 1) fused2_kernel(Fused2Args ga) {
+    using C = F2Cfg<LA, LB, LC, LD, PURE, PB, NCH>;
+    using I = F2Impl<LA, LB, LC, LD, PURE, PB, NCH>;
+    constexpr int L = C::L;
+    const FusedArgs &g = ga.f;
+    extern __shared__ double sm[];
+    const int NQ = ga.NQ, NC = NCH * ga.TCH, NT = blockDim.x, NP = NT - NC;
+    // carve-up: [NQ] x { sidx[4 ints], obase, pad, BT, EPB, half } then 2 x [NQ] x batch record
+    double *perq = sm;
+    double *batch = sm + (size_t)NQ * C::PERQ;
+    unsigned *packq = (unsigned *)(batch + (size_t)2 * NQ * C::BREC);     // [EPK]  ket product words
+    unsigned *packc = packq + even_up(C::EPK);                             // [NPB]  bra product words
+    constexpr int O_OB = 2, O_BT = 4, O_EPB = O_BT + C::TB, O_HALF = O_EPB + even_up(C::NPB);
+    const int tid = threadIdx.x;
+    const bool consumer = tid < NC;
+    const int ptid = tid - NC;
+    const int Ka = g.bra.a.K, Kb = g.bra.single ? 1 : g.bra.b.K;
+    const int Kc = g.ket.a.K, Kd = g.ket.single ? 1 : g.ket.b.K;
+    const int Kbra = Ka * Kb, Kket = Kc * Kd;
+
+    // consumer role: chunk ch, quartet slot cj, Hermite rows ip[k]
+    int ch = 0, cj = 0, ip[PB], pofs[PB];
+    bool cact = false;
+    if (consumer) {
+        ch = tid / ga.TCH;
+        const int r = tid - ch * ga.TCH;
+        cact = r < NQ * C::NPG;
+        cj = r / C::NPG;
+        const int pg = r - cj * C::NPG;
+#pragma unroll
+        for (int k = 0; k < PB; ++k) {
+            const int i = d_pmap<C::Lb, PB, L>.p[k][pg];
+            ip[k] = cact ? i : -1;
+            const int w = d_herm<C::NHB>.e[i < 0 ? 0 : i];
+            pofs[k] = C::BR.A * (w & 0xff) + C::BR.B * (w >> 8 & 0xff) + (w >> 16);
+        }
+    }
+
+    for (int e = tid; e < C::EPK; e += NT) packq[e] = d_packq<LC, LD, NCH>.w[e];
+    for (int e = tid; e < C::NPB; e += NT) packc[e] = d_packc<LA, LB>.w[e];
+
+    const long long ngroups = (g.nq + NQ - 1) / NQ;
+    for (long long grp = blockIdx.x; grp < ngroups; grp += gridDim.x) {
+        const long long q0 = grp * NQ;
+        const int nqg = (int)min((long long)NQ, g.nq - q0);
+        __syncthreads();                                     // previous group is done with shared memory
+        if (tid < nqg) {
+            const long long q = q0 + tid;
+            long long bi, ki;
+            if (g.qidx) { bi = g.qidx[2 * q]; ki = g.qidx[2 * q + 1]; }
+            else { bi = q / g.nket; ki = q % g.nket; }
+            long long ia = bi, ib = bi, ic = ki, id = ki;
+            if (g.bra.idx) { ia = g.bra.idx[2 * bi + g.bra_swap]; ib = g.bra.idx[2 * bi + 1 - g.bra_swap]; }
+            if (g.ket.idx) { ic = g.ket.idx[2 * ki + g.ket_swap]; id = g.ket.idx[2 * ki + 1 - g.ket_swap]; }
+            double *pq = perq + (size_t)tid * C::PERQ;
+            int *sidx = (int *)pq;
+            sidx[0] = (int)ia; sidx[1] = (int)ib; sidx[2] = (int)ic; sidx[3] = (int)id;
+            *(long long *)(pq + O_OB) = q * g.s_q + bi * g.s_bi + ki * g.s_ki;
+        }
+        __syncthreads();
+
+        for (int kb = 0; kb < Kbra; ++kb) {
+            if (consumer) {
+                // ---------------- consumers: P4 over the ket primitives ----------------
+                double hacc[PB][C::NACC];
+#pragma unroll
+                for (int k = 0; k < PB; ++k)
+#pragma unroll
+                    for (int i = 0; i < C::NACC; ++i) hacc[k][i] = 0.0;
+                for (int kk = 0; kk < Kket; ++kk) {
+                    const int buf = kk & 1;
+                    bar_sync(F2_BAR_FULL + buf, NC + NP / 2);
+                    if (cact && cj < nqg) {
+                        const double *rec = batch + ((size_t)buf * NQ + cj) * C::BREC;
+                        const double *Rb = rec + C::O_A;
+                        const double *EP = rec + C::O_EP;
+                        if (NCH == 1 || ch == 0) f2_contract<C, LC, LD, PB, NCH, 0>(hacc, Rb, pofs, EP);
+                        if constexpr (NCH > 1) { if (ch == 1) f2_contract<C, LC, LD, PB, NCH, 1>(hacc, Rb, pofs, EP); }
+                        if constexpr (NCH > 2) { if (ch == 2) f2_contract<C, LC, LD, PB, NCH, 2>(hacc, Rb, pofs, EP); }
+                    }
+                    if (kk + 2 < Kket) bar_arrive(F2_BAR_EMPTY + buf, NC + NP / 2);
+                }
+                if (cact && cj < nqg)
+                    f2_flush<C, LD, PURE, PB>(hacc, ch * C::CHC, ip, perq + (size_t)cj * C::PERQ + O_HALF);
+            } else {
+                // ---------------- producers: tables, Boys, Hermite Coulomb tensors ----------------
+                // Two producer groups work on alternate ket primitives (group g fills buffer g), so that
+                // each has two consumer batches of time for its four dependent stages.
+                for (int it = ptid; it < 3 * nqg; it += NP) {             // bra tables of primitive kb
+                    const int j = it / 3, ax = it - 3 * j;
+                    double *pq = perq + (size_t)j * C::PERQ;
+                    const int *sidx = (const int *)pq;
+                    table_task<LA, LB>(g.bra, sidx[0], sidx[1], kb / Kb, kb % Kb, ax, pq + O_BT);
+                }
+                bar_sync(F2_BAR_PALL, NP);
+                const int NG = NP / 2, pgp = ptid / NG, gt = ptid - pgp * NG;
+                double *brec = batch + (size_t)pgp * NQ * C::BREC;
+                for (int kk = pgp; kk < Kket; kk += 2) {
+                    if (kk >= 2) bar_sync(F2_BAR_EMPTY + pgp, NC + NG);
+                    for (int it = gt; it < 3 * nqg; it += NG) {           // stage 0: ket tables of primitive kk
+                        const int j = it / 3, ax = it - 3 * j;
+                        const int *sidx = (const int *)(perq + (size_t)j * C::PERQ);
+                        table_task<LC, LD>(g.ket, sidx[2], sidx[3], kk / Kd, kk % Kd, ax, brec + (size_t)j * C::BREC + C::O_TK);
+                    }
+                    bar_sync(F2_BAR_PROD + pgp, NG);
+                    if (gt < nqg) {                                       // stage 1a: Boys, [0]^(m), z-line
+                        I::z_task(perq + (size_t)gt * C::PERQ + O_BT, brec + (size_t)gt * C::BREC, g.boys_tab);
+                    } else if (gt >= NQ) {                                // stage 1b: ket products, q~-major
+                        const int nw = NG - NQ, w = gt - NQ;
+                        for (int j = 0; j < nqg; ++j) {
+                            double *rec = brec + (size_t)j * C::BREC;
+#pragma unroll 4
+                            for (int e = w; e < C::EPK; e += nw) rec[C::O_EP + e] = prod_entry(rec + C::O_TK, packq[e]);
+                        }
+                    }
+                    bar_sync(F2_BAR_PROD + pgp, NG);
+                    for (int it = gt; it < (L + 1) * nqg; it += NG) {     // stage y (tasks sorted by line length)
+                        const int v = it / nqg, j = it - v * nqg;
+                        I::y_task(v, brec + (size_t)j * C::BREC);
+                    }
+                    bar_sync(F2_BAR_PROD + pgp, NG);
+                    for (int it = gt; it < C::NZ * nqg; it += NG) {       // stage x (sorted by line length)
+                        int c = it / nqg;
+                        const int j = it - c * nqg;
+                        int s = 0;
+                        while (c > s) { c -= s + 1; ++s; }                // column c of the anti-diagonal u+v = s
+                        I::x_task(c, s - c, brec + (size_t)j * C::BREC);
+                    }
+                    bar_arrive(F2_BAR_FULL + pgp, NC + NG);
+                }
+                // bra products of primitive kb (component-major list for P5)
+                for (int j = 0; j < nqg; ++j) {
+                    double *pq = perq + (size_t)j * C::PERQ;
+#pragma unroll 4
+                    for (int e = ptid; e < C::NPB; e += NP) pq[O_EPB + e] = prod_entry(pq + O_BT, packc[e]);
+                }
+            }
+            __syncthreads();                                 // [p~|c md] rows and bra products are in place
+            if constexpr (PURE && LC > 0) {                  // ket c-index transform, in place per (p~, md)
+                constexpr SolidTab<LC> S{};
+                for (int it = tid; it < nqg * C::NHB * C::NDO; it += NT) {
+                    const int j = it / (C::NHB * C::NDO), r = it - j * (C::NHB * C::NDO), p = r / C::NDO, md = r - p * C::NDO;
+                    double *row = perq + (size_t)j * C::PERQ + O_HALF + p * C::HS + md;
+                    double x[C::NCC];
+#pragma unroll
+                    for (int c = 0; c < C::NCC; ++c) x[c] = row[c * C::NDO];
+#pragma unroll
+                    for (int m = 0; m < C::NCO; ++m) {
+                        double s = 0.0;
+#pragma unroll
+                        for (int c = 0; c < C::NCC; ++c)
+                            if (S.c[m][c] != 0.0) s = fma(S.c[m][c], x[c], s);
+                        row[m * C::NDO] = s;
+                    }
+                }
+                __syncthreads();
+            }
+            // P5: [ab|cd] += sum_p~ E^{ab}_{p~} [p~|cd]  (Eq. 26), bra transform, accumulate in the output
+            for (int it = tid; it < nqg * C::NCD_O; it += NT) {
+                const int j = it / C::NCD_O, icd = it - j * C::NCD_O;
+                const double *pq = perq + (size_t)j * C::PERQ;
+                const double *half = pq + O_HALF + icd;
+                double hv[C::NHB];
+#pragma unroll
+                for (int i = 0; i < C::NHB; ++i) hv[i] = half[i * C::HS];
+                double oacc[C::NAB_C];
+#pragma unroll
+                for (int i = 0; i < C::NAB_C; ++i) oacc[i] = 0.0;
+                const double2 *ep = (const double2 *)(pq + O_EPB);
+                constexpr ProdList<LA, LB, 0> PBL{};
+                double2 e2 = make_double2(0.0, 0.0);
+                static_for<PBL.N>([&](auto ic) {
+                    constexpr int i = decltype(ic)::value;
+                    if constexpr ((i & 1) == 0) e2 = ep[i / 2];
+                    oacc[PBL.comp[i]] = fma((i & 1) ? e2.y : e2.x, hv[PBL.off[i]], oacc[PBL.comp[i]]);
+                });
+                double o2[C::NAB_O];
+                solid2<LA, LB, PURE>(oacc, o2);
+                double *o = g.out + *(const long long *)(pq + O_OB) + (icd / C::NDO) * g.sc + (icd % C::NDO) * g.sd;
+                if (kb == 0) {
+#pragma unroll
+                    for (int a = 0; a < C::NAO; ++a)
+#pragma unroll
+                        for (int b = 0; b < C::NBO; ++b) o[a * g.sa + b * g.sb] = o2[a * C::NBO + b];
+                } else {
+#pragma unroll
+                    for (int a = 0; a < C::NAO; ++a)
+#pragma unroll
+                        for (int b = 0; b < C::NBO; ++b) o[a * g.sa + b * g.sb] += o2[a * C::NBO + b];
+                }
+            }
+            __syncthreads();                                 // rows, products and tables may be rewritten
+        }
+    }
+}
+
+}  // namespace mdb

@@ -13,4 +13,10 @@ static inline cudaError_t fused_init(int max_smem) { return fused_register_all(m
 int fused_dispatch(const PairView &b, const PairView &k, long long nq, const int32_t *qidx, int pure, int layout,
                    double *out, const double *boys_tab, int nsm, cudaStream_t st, bool force);
 
+// Warp-specialised fused kernels (fused2_inst.cu): same contract as fused_dispatch; info (may be null)
+// receives {PB, NCH, NQ, consumer threads, smem bytes}.
+cudaError_t fused2_init(int max_smem);
+int fused2_dispatch(const PairView &b, const PairView &k, long long nq, const int32_t *qidx, int pure, int layout,
+                    double *out, const double *boys_tab, int nsm, cudaStream_t st, int *info);
+
 }  // namespace mdb

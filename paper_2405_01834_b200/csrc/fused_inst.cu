@@ -48,15 +48,14 @@ cudaError_t fused_register_all(int max_smem) {
 
 namespace mdb {
 
-int fused_dispatch(const PairView &b0, const PairView &k0, long long nq, const int32_t *qidx, int pure, int layout,
-                   double *out, const double *boys_tab, int nsm, cudaStream_t st, bool /*force*/) {
+// Canonical order (la >= lb, lc >= ld) and output strides for a fused launch; l[] receives the kernel's class.
+void fused_make_args(const PairView &b0, const PairView &k0, long long nq, const int32_t *qidx, int pure, int layout,
+                     double *out, const double *boys_tab, FusedArgs &g, int l[4]) {
     PairView b = b0, k = k0;
     int la = b.a.l, lb = b.single ? 0 : b.b.l, lc = k.a.l, ld = k.single ? 0 : k.b.l;
-    if (la > MD_FUSED_LMAX || lb > MD_FUSED_LMAX || lc > MD_FUSED_LMAX || ld > MD_FUSED_LMAX) return 0;
     // caller's component strides (include/md_b200.h layouts)
     const long long na = ncomp(la, pure), nb = ncomp(lb, pure), nc = ncomp(lc, pure), nd = ncomp(ld, pure);
     const long long nab = na * nb, ncd = nc * nd;
-    FusedArgs g;
     long long ca, cb, cc, cd;
     if (layout == 1) {                               // MD_LAYOUT_PAPER: ij + nbra*(ab + N_ab*(cd + N_cd*kl))
         const long long nbra = b.npairs;
@@ -70,11 +69,22 @@ int fused_dispatch(const PairView &b0, const PairView &k0, long long nq, const i
     g.bra_swap = 0; g.ket_swap = 0;
     if (!b.single && la < lb) { std::swap(b.a, b.b); std::swap(la, lb); std::swap(ca, cb); g.bra_swap = 1; }
     if (!k.single && lc < ld) { std::swap(k.a, k.b); std::swap(lc, ld); std::swap(cc, cd); g.ket_swap = 1; }
-    const FusedEntry &e = g_table[(((la * 3 + lb) * 3 + lc) * 3 + ld) * 2 + (pure ? 1 : 0)];
-    if (!e.fn) return 0;
     g.bra = b; g.ket = k; g.qidx = qidx; g.nq = nq; g.nket = k.npairs; g.out = out;
     g.sa = ca; g.sb = cb; g.sc = cc; g.sd = cd;
     g.boys_tab = boys_tab; g.rlut = g_rlut;
+    l[0] = la; l[1] = lb; l[2] = lc; l[3] = ld;
+}
+
+int fused_dispatch(const PairView &b0, const PairView &k0, long long nq, const int32_t *qidx, int pure, int layout,
+                   double *out, const double *boys_tab, int nsm, cudaStream_t st, bool /*force*/) {
+    if (b0.a.l > MD_FUSED_LMAX || (!b0.single && b0.b.l > MD_FUSED_LMAX) || k0.a.l > MD_FUSED_LMAX ||
+        (!k0.single && k0.b.l > MD_FUSED_LMAX))
+        return 0;
+    FusedArgs g;
+    int l[4];
+    fused_make_args(b0, k0, nq, qidx, pure, layout, out, boys_tab, g, l);
+    const FusedEntry &e = g_table[(((l[0] * 3 + l[1]) * 3 + l[2]) * 3 + l[3]) * 2 + (pure ? 1 : 0)];
+    if (!e.fn) return 0;
     const long long ngroups = (nq + e.nq - 1) / e.nq;
     const unsigned grid = (unsigned)std::min<long long>(ngroups, (long long)nsm * e.ctas_per_sm);
     e.fn<<<grid, MD_FUSED_THREADS, e.smem, st>>>(g);

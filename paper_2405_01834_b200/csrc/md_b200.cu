@@ -32,6 +32,7 @@ struct State {
     int last_variant = 0;
     int last_launches = 0;
     int last_mma_info[8] = {0};
+    int last_f2_info[8] = {0};
     int nsm = 148;
     int max_smem = 227 * 1024;
     char cuda_err[256] = "";
@@ -226,7 +227,21 @@ int run(const PairView &b, const PairView &k, long long nq, const int32_t *qidx,
     if (e) return e;
     S.last_launches = 0;
     if (nq == 0) return MD_OK;
-    if (S.variant == MD_VARIANT_AUTO || S.variant == MD_VARIANT_FUSED) {
+    if (S.variant == MD_VARIANT_AUTO || S.variant == MD_VARIANT_FUSED2) {
+        // contracted classes: the warp-specialised kernel amortises its pipeline over the primitive loop
+        const long long nprim = (long long)b.a.K * (b.single ? 1 : b.b.K) * k.a.K * (k.single ? 1 : k.b.K);
+        if (S.variant == MD_VARIANT_FUSED2 || nprim >= 4) {
+            int r = fused2_dispatch(b, k, nq, qidx, pure, layout, out, S.boys_tab, S.nsm, st, S.last_f2_info);
+            if (r == 1) {
+                S.last_launches++;
+                CK(cudaGetLastError());
+                S.last_variant = MD_VARIANT_FUSED2;
+                return MD_OK;
+            }
+            if (r < 0) return r;
+        }
+    }
+    if (S.variant == MD_VARIANT_AUTO || S.variant == MD_VARIANT_FUSED || S.variant == MD_VARIANT_FUSED2) {
         int r = fused_dispatch(b, k, nq, qidx, pure, layout, out, S.boys_tab, S.nsm, st, S.variant == MD_VARIANT_FUSED);
         if (r == 1) {
             S.last_launches++;
@@ -265,6 +280,7 @@ int md_init(void) {
     CK(cudaFuncSetAttribute(eri_generic_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, S.max_smem - 1024));
     CK(cudaFuncSetAttribute(pair_setup_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, 96 * 1024));
     CK(fused_init(S.max_smem));
+    CK(fused2_init(S.max_smem));
     CK(mma_init(S.max_smem));
     CK(cudaDeviceSynchronize());
     S.init = true;
@@ -317,7 +333,7 @@ int md_set_workspace(void *p, size_t bytes) {
     return MD_OK;
 }
 int md_set_variant(int v) {
-    if (v < MD_VARIANT_AUTO || v > MD_VARIANT_MMA) return MD_EINVAL;
+    if (v < MD_VARIANT_AUTO || v > MD_VARIANT_FUSED2) return MD_EINVAL;
     S.variant = v;
     return MD_OK;
 }
