@@ -120,6 +120,51 @@ def test_config2_dddd_K1_and_K3_sampled():
             check(w, pure)
 
 
+# ---- the warp-specialised fused kernel (fused2) -------------------------------------------------------------
+
+FUSED2 = engine.VARIANT_FUSED2
+
+
+@pytest.mark.parametrize("K", [1, 2, 3])
+def test_fused2_config2_dddd(K):
+    """(dd|dd): the kernel bench.py times, on config-2 inputs, both outputs, a ragged quartet count."""
+    w = W.config2(K=K, n=613)
+    for pure in (True, False):
+        _, used = check(w, pure, FUSED2)
+        assert used == FUSED2
+
+
+@pytest.mark.parametrize("n", [1, 2, 7, 8, 9, 151])
+def test_fused2_tails_and_small_batches(n):
+    """Fewer quartets than one CTA pass, one more than a pass, and a count that leaves most CTAs idle."""
+    w = W.independent_quartets("f2tail", (2, 2, 2, 2), (2, 3, 1, 2), n, (0.05, 50.0), (-2.0, 2.0), W.class_seed("f2tail", n))
+    for pure in (True, False):
+        _, used = check(w, pure, FUSED2)
+        assert used == FUSED2
+
+
+def test_fused2_mixed_contraction_and_clustered():
+    for Ks in [(3, 1, 1, 3), (1, 4, 2, 1), (5, 1, 1, 1), (1, 1, 1, 6)]:
+        w = W.independent_quartets("f2mix", (2, 2, 2, 2), Ks, 41, (0.05, 50.0), (-3.0, 3.0), W.class_seed("f2mix", Ks))
+        check(w, True, FUSED2)
+        check(w, False, FUSED2)
+    for coincide in (None, "AB", "CD", "ALL"):
+        check(W.clustered((2, 2, 2, 2), 29, K=(2, 2, 2, 2), coincide=coincide), True, FUSED2)
+
+
+def test_fused2_product_mode_and_paper_layout():
+    w = _product((2, 2, 2, 2), 11, 6, K=3)
+    for pure in (True, False):
+        ref = oracle_run(w, pure)
+        gpu, used = gpu_run(w, pure, FUSED2)
+        assert used == FUSED2
+        assert_parity(gpu.reshape(ref.shape), ref, "fused2 product")
+        gp, _ = gpu_run(w, pure, FUSED2, layout=engine.LAYOUT_PAPER)
+        n = engine.ncomp(2, pure) ** 2
+        v = gp.reshape(6, n, n, 11).transpose(3, 0, 2, 1).reshape(11 * 6, n * n)
+        assert_parity(v, ref, "fused2 paper layout")
+
+
 # ---- 3-center ----------------------------------------------------------------------------------------------
 
 @pytest.mark.parametrize("la,lb,lX", [(0, 0, 0), (1, 0, 0), (0, 1, 2), (1, 1, 1), (2, 2, 2), (2, 0, 6), (3, 3, 6), (3, 1, 4),
