@@ -117,6 +117,15 @@ def cpu_baseline(K, pure, nsample):
             "sample": f"first {nsample} of the {NQ} quartets, {dt:.1f} s, gcc -O2 OpenMP over quartets"}, dt
 
 
+def ncu_traffic(variant):
+    """dram__bytes_read.sum + dram__bytes_write.sum per launch of the timed kernel, from the committed
+    ncu --set full capture of this workload (profiles/traffic.json), or None if there is none."""
+    try:
+        return json.load(open(os.path.join(ROOT, "profiles", "traffic.json"))).get(variant)
+    except (OSError, ValueError):
+        return None
+
+
 def run_reference(args):
     rank = int(os.environ.get("RANK", "0"))
     if rank != 0:
@@ -155,7 +164,7 @@ def run_ours(args):
     import numpy as np
     import torch
     import torch.distributed as dist
-    from paper_2405_01834_b200 import build, engine, workloads as W
+    from paper_2405_01834_b200 import build, engine, sharding, workloads as W
 
     rank = int(os.environ.get("RANK", "0"))
     local = int(os.environ.get("LOCAL_RANK", "0"))
@@ -177,10 +186,7 @@ def run_ours(args):
         head = measure_variant(dw, w, K, pure, args.steps, args.warmup, flush, barrier)
     clocks = cs.summary()
     ms_total = head["ms_per_step"] * args.steps
-    if world > 1:
-        t = torch.tensor([ms_total], dtype=torch.float64, device="cuda")
-        dist.all_reduce(t, op=dist.ReduceOp.MAX)
-        ms_total = float(t.item())
+    ms_total = sharding.max_over_ranks(ms_total, "cuda")
     value = world * w.nquartets * args.steps / (ms_total * 1e-3)
 
     # end to end: the host-buffer C-ABI call, pinned host memory, copies inside the timed region
@@ -209,10 +215,7 @@ def run_ours(args):
         e2e_step()
     torch.cuda.synchronize(); barrier()
     e2e_s = time.perf_counter() - t0
-    if world > 1:
-        t = torch.tensor([e2e_s], dtype=torch.float64, device="cuda")
-        dist.all_reduce(t, op=dist.ReduceOp.MAX)
-        e2e_s = float(t.item())
+    e2e_s = sharding.max_over_ranks(e2e_s, "cuda")
     e2e_val = world * w.nquartets * esteps / e2e_s
 
     line = {"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
@@ -233,12 +236,12 @@ def run_ours(args):
         dmma_tf, _ = engine.md_fp64_peak(1, 0.3)
         achieved = head["model_tflops"]
         line["roofline"] = {"bound": "alu", "achieved": achieved, "peak": FP64_PEAK_DERIVED_TFLOPS, "unit": "TFLOP/s",
-                            "frac": achieved / FP64_PEAK_DERIVED_TFLOPS, "traffic": None,
+                            "frac": achieved / FP64_PEAK_DERIVED_TFLOPS, "traffic": ncu_traffic(head["variant"]),
                             "peak_source": "derived: 148 SM x 64 DFMA/clk x 2 x 1.965 GHz (DESIGN.md)",
                             "peak_measured_dfma_loop": dfma_tf, "peak_measured_dmma_m8n8k4_loop": dmma_tf,
                             "frac_of_measured_dfma": achieved / dfma_tf if dfma_tf else None,
                             "algorithmic_flop_per_quartet": head["model_flop_per_quartet"],
-                            "kernel": "md_eri4 step (all launches of the call)",
+                            "kernel": f"md_eri4 step = {head['launches_per_step']} launch(es) of the {head['variant']} kernel",
                             "hbm_gbs_algorithmic": (head["out_bytes"] + h2d) / (head["ms_per_step"] * 1e-3) / 1e9}
         try:
             peaks = json.load(open(os.path.join(ROOT, "MEASURED_PEAKS.json")))
