@@ -45,20 +45,31 @@ struct F2Cfg {
     static constexpr int HW = NCC * NDO;                       // [c][md] before the c transform
     static constexpr int HS = HW | 1;                          // odd row stride: conflict-free columns
     static constexpr int NZ = (L + 1) * (L + 2) / 2;           // entries of the z-line output
-    // one batch record per quartet (doubles)
     static constexpr Brick BR = brick_layout(L, Lb);
     static_assert(brick_injective(L, BR), "brick layout must be injective");
     static constexpr int NRA = even_up(BR.foot > NZ ? BR.foot : NZ);
-    static constexpr int O_A = 0;                              // z-line output, later [r]^(0) in the brick layout
-    static constexpr int O_B = O_A + NRA;                      // [0uv]^(m) columns
+    // consumer-visible buffer of one quartet and batch (doubles): what P4 reads
+    static constexpr int O_R = 0;                              // z-line output, later [r]^(0) in the brick layout
+    static constexpr int O_EP = NRA;                           // ket product list
+    static constexpr int CB = O_EP + even_up(EPK);
+    static constexpr int NBUF = 4;                             // two per producer group
+    // producer-group scratch of one quartet: only live while a batch is being built
+    static constexpr int O_B = 0;                              // [0uv]^(m) columns
     static constexpr int O_PQ = O_B + even_up(NHL);            // X, Y, Z, pad
     static constexpr int O_TK = O_PQ + 4;                      // ket table record
-    static constexpr int O_EP = O_TK + TK;                     // ket product list
-    static constexpr int BREC = O_EP + even_up(EPK);
-    // per quartet, outside the batch buffers
-    static constexpr int PERQ = 2 /*sidx*/ + 2 /*out base, flags*/ + TB + even_up(NPB) + NHB * HS + (NHB * HS & 1);
+    // strides between quartets are 2 mod 4 doubles: lanes that do the same task for 8 consecutive quartets
+    // then fall on 8 distinct 8-byte banks
+    static constexpr int pad_bank(int x) { return x + ((2 - x) % 4 + 4) % 4; }
+    static constexpr int GS = pad_bank(O_TK + TK);
+    static constexpr int CBQ = pad_bank(NBUF * CB);             // the NBUF buffers of one quartet
+    // drain region of one quartet, aliased on its NBUF buffers once every batch of the bra primitive is consumed
+    static constexpr int O_HALF = 0, O_EPB = even_up(NHB * HS);
+    static_assert(O_EPB + even_up(NPB) <= NBUF * CB, "drain region must fit in the batch buffers");
+    // per quartet, never aliased: shell indices, output base, bra table record
+    static constexpr int PERQ = 4 + TB;
+    static constexpr int QTOT = PERQ + CBQ + 2 * GS;
     static constexpr int FIXED = (even_up(EPK) + even_up(NPB)) / 2;    // packed product words (doubles)
-    static __host__ __device__ constexpr size_t smem_bytes(int nq) { return 8 * ((size_t)nq * (PERQ + 2 * BREC) + FIXED); }
+    static __host__ __device__ constexpr size_t smem_bytes(int nq) { return 8 * ((size_t)nq * QTOT + FIXED); }
 };
 
 __device__ __forceinline__ void bar_sync(int id, int n) { asm volatile("bar.sync %0, %1;" ::"r"(id), "r"(n) : "memory"); }
@@ -66,7 +77,7 @@ __device__ __forceinline__ void bar_arrive(int id, int n) {
     __threadfence_block();
     asm volatile("bar.arrive %0, %1;" ::"r"(id), "r"(n) : "memory");
 }
-enum { F2_BAR_PALL = 1, F2_BAR_FULL = 2, F2_BAR_EMPTY = 4, F2_BAR_PROD = 6 };
+enum { F2_BAR_PALL = 1, F2_BAR_PROD = 2, F2_BAR_CONS = 4, F2_BAR_FULL = 5, F2_BAR_EMPTY = 9 };   // FULL/EMPTY: 4 ids each
 
 // One axis of the two-centre table, written compactly (rows (i,j), t = 0..i+j).
 template <int L1, int L2>
@@ -82,7 +93,8 @@ __device__ __forceinline__ void axis_table_compact(double za, double zb, double 
             for (int t = 0; t <= i + j; ++t) E[e1_rowoff(L2, i, j) + t] = tmp[(i * (L2 + 1) + j) * NT + t];
 }
 
-// Table record of one primitive pair: rec[0] = p, rec[1..3] = P, rec[4] = c_a c_b, rec[8 + ax*E1 + ..].
+// Table record of one primitive pair: rec[0] = p, rec[1..3] = P, rec[4] = c_a c_b, rec[5] = -c_a c_b,
+// rec[6] = 0, rec[8 + ax*E1 + ..] = the compact 1-D tables (the slots prod_word addresses).
 template <int L1, int L2>
 __device__ __forceinline__ void table_task(const PairView &pv, long long i1, long long i2, int k1, int k2, int ax, double *rec) {
     constexpr int E1 = e1_count(L1, L2);
@@ -95,7 +107,8 @@ __device__ __forceinline__ void table_task(const PairView &pv, long long i1, lon
     rec[1 + ax] = (za * A + zb * B) / p;
     if (ax == 0) {
         rec[0] = p;
-        rec[4] = __ldg(pv.a.coefs + i1 * K1 + k1) * (pv.single ? 1.0 : __ldg(pv.b.coefs + i2 * K2 + k2));
+        const double c = __ldg(pv.a.coefs + i1 * K1 + k1) * (pv.single ? 1.0 : __ldg(pv.b.coefs + i2 * K2 + k2));
+        rec[4] = c; rec[5] = -c; rec[6] = 0.0; rec[7] = 0.0;
     }
 }
 
@@ -127,8 +140,8 @@ struct F2Impl {
 
     // ---- producer stages -------------------------------------------------------------------
     // stage 1a: Boys function, [0]^(m) and the z-line for one tensor
-    static __device__ __forceinline__ void z_task(const double *bt, double *rec, const double *boys_tab) {
-        const double *kt = rec + C::O_TK;
+    static __device__ __forceinline__ void z_task(const double *bt, double *gs, double *cb, const double *boys_tab) {
+        const double *kt = gs + C::O_TK;
         const double p = bt[0], q = kt[0];
         const double X = bt[1] - kt[1], Y = bt[2] - kt[2], Z = bt[3] - kt[3];
         const double rho = p * q / (p + q);
@@ -139,8 +152,8 @@ struct F2Impl {
         const double m2r = -2.0 * rho;
 #pragma unroll
         for (int m = 0; m <= L; ++m) { a[0][m] = F[m] * f; f *= m2r; a[1][m] = 0.0; }
-        rec[C::O_PQ] = X; rec[C::O_PQ + 1] = Y; rec[C::O_PQ + 2] = Z;
-        double *zo = rec + C::O_A;
+        gs[C::O_PQ] = X; gs[C::O_PQ + 1] = Y; gs[C::O_PQ + 2] = Z;
+        double *zo = cb + C::O_R;
         line_recursion<L>(Z, a, L, [&](auto vc, double(&row)[L + 1]) {
             constexpr int v = decltype(vc)::value;
             constexpr int off = v * (L + 1) - v * (v - 1) / 2;
@@ -149,14 +162,14 @@ struct F2Impl {
         });
     }
     // stage y: thread owns v; [0uv]^(m) for u = 0..L-v, written as columns (u,v) of L-u-v+1 entries
-    static __device__ __forceinline__ void y_task(int v, double *rec) {
+    static __device__ __forceinline__ void y_task(int v, double *gs, const double *cb) {
         const int n = L - v;
-        const double *zo = rec + C::O_A + v * (L + 1) - v * (v - 1) / 2;
+        const double *zo = cb + C::O_R + v * (L + 1) - v * (v - 1) / 2;
         double a[2][L + 1];
 #pragma unroll
         for (int m = 0; m <= L; ++m) { a[0][m] = m <= n ? zo[m] : 0.0; a[1][m] = 0.0; }
-        double *col = rec + C::O_B + (nherm(L) - nherm(n));                // block of this v
-        line_recursion<L>(rec[C::O_PQ + 1], a, n, [&](auto uc, double(&row)[L + 1]) {
+        double *col = gs + C::O_B + (nherm(L) - nherm(n));                 // block of this v
+        line_recursion<L>(gs[C::O_PQ + 1], a, n, [&](auto uc, double(&row)[L + 1]) {
             constexpr int u = decltype(uc)::value;
 #pragma unroll
             for (int m = 0; m <= L - u; ++m)
@@ -165,14 +178,14 @@ struct F2Impl {
         });
     }
     // stage x: thread owns the line (u,v); emits [tuv]^(0) into the brick layout (fused2_tables.cuh)
-    static __device__ __forceinline__ void x_task(int u, int v, double *rec) {
+    static __device__ __forceinline__ void x_task(int u, int v, const double *gs, double *cb) {
         const int nv = L - v, n = nv - u;
-        const double *col = rec + C::O_B + (nherm(L) - nherm(nv)) + u * (nv + 1) - u * (u - 1) / 2;
+        const double *col = gs + C::O_B + (nherm(L) - nherm(nv)) + u * (nv + 1) - u * (u - 1) / 2;
         double a[2][L + 1];
 #pragma unroll
         for (int m = 0; m <= L; ++m) { a[0][m] = m <= n ? col[m] : 0.0; a[1][m] = 0.0; }
-        double *R = rec + C::O_A + C::BR.B * u + v;
-        line_recursion<L>(rec[C::O_PQ], a, n, [&](auto tc, double(&row)[L + 1]) {
+        double *R = cb + C::O_R + C::BR.B * u + v;
+        line_recursion<L>(gs[C::O_PQ], a, n, [&](auto tc, double(&row)[L + 1]) {
             constexpr int t = decltype(tc)::value;
             R[C::BR.A * t] = row[0];
         });

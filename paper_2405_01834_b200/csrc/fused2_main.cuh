@@ -6,6 +6,7 @@ namespace mdb {
 
 struct Fused2Args {
     FusedArgs f;                  // shells, index lists, output strides (as for fused_kernel)
+    double *scratch;              // per-CTA pair-table scratch (stays in L2): [grid][NQ][Kbra*TB + Kket*TK]
     int NQ;                       // quartets per CTA pass
     int TCH;                      // consumer threads per cd chunk (multiple of 32, >= NQ*NPG)
 };
@@ -53,9 +54,35 @@ __device__ __forceinline__ void f2_contract(double (&hacc)[PB][C::NACC], const d
 
 // One product-list entry from a table record and its packed word (fused2_tables.cuh).
 __device__ __forceinline__ double prod_entry(const double *tab, unsigned w) {
-    double v = tab[4] * tab[w & 1023] * (tab[w >> 10 & 1023] * tab[w >> 20 & 1023]);
-    if (w >> 30 & 1) v = -v;
-    return (w >> 31) ? v : 0.0;
+    return (tab[w & 255] * tab[w >> 8 & 255]) * (tab[w >> 16 & 255] * tab[w >> 24]);
+}
+
+// n products of one table record, entries w, w + stride, ...: all loads of a batch of four entries are
+// issued before the first store (the compiler cannot reorder them itself: same shared array).
+__device__ __forceinline__ void prod_list(const double *tab, const unsigned *pack, double *dst, int n, int w, int stride) {
+    for (int e0 = w; e0 < n; e0 += 4 * stride) {
+        unsigned ww[4];
+        double v[4];
+#pragma unroll
+        for (int u = 0; u < 4; ++u) ww[u] = e0 + u * stride < n ? pack[e0 + u * stride] : PROD_WORD_ZERO;
+#pragma unroll
+        for (int u = 0; u < 4; ++u) v[u] = prod_entry(tab, ww[u]);
+#pragma unroll
+        for (int u = 0; u < 4; ++u)
+            if (e0 + u * stride < n) dst[e0 + u * stride] = v[u];
+    }
+}
+
+// Copy n doubles global -> shared, eight loads in flight per thread.
+__device__ __forceinline__ void copy_in(double *dst, const double *src, int n, int t, int nt) {
+    for (int i0 = t; i0 < n; i0 += 8 * nt) {
+        double v[8];
+#pragma unroll
+        for (int u = 0; u < 8; ++u) v[u] = i0 + u * nt < n ? __ldcg(src + i0 + u * nt) : 0.0;
+#pragma unroll
+        for (int u = 0; u < 8; ++u)
+            if (i0 + u * nt < n) dst[i0 + u * nt] = v[u];
+    }
 }
 
 // Flush of one chunk: ket d-index transform in registers (Eq. 16), rows to shared memory.
@@ -95,18 +122,24 @@ __global__ void __launch_bounds__(MD_F2_PRODUCERS + 192, 1) fused2_kernel(Fused2
     const FusedArgs &g = ga.f;
     extern __shared__ double sm[];
     const int NQ = ga.NQ, NC = NCH * ga.TCH, NT = blockDim.x, NP = NT - NC;
-    // carve-up: [NQ] x { sidx[4 ints], obase, pad, BT, EPB, half } then 2 x [NQ] x batch record
+    // carve-up: [NQ] x { sidx[4 ints], obase, pad, BT }, [NQ] x NBUF consumer buffers (the drain region
+    // {half, EPB} of a quartet aliases its buffers), 2 x [NQ] producer-group scratch, packed product words
     double *perq = sm;
-    double *batch = sm + (size_t)NQ * C::PERQ;
-    unsigned *packq = (unsigned *)(batch + (size_t)2 * NQ * C::BREC);     // [EPK]  ket product words
+    double *bufs = sm + (size_t)NQ * C::PERQ;
+    double *gsc = bufs + (size_t)NQ * C::CBQ;
+    unsigned *packq = (unsigned *)(gsc + (size_t)2 * NQ * C::GS);          // [EPK]  ket product words
     unsigned *packc = packq + even_up(C::EPK);                             // [NPB]  bra product words
-    constexpr int O_OB = 2, O_BT = 4, O_EPB = O_BT + C::TB, O_HALF = O_EPB + even_up(C::NPB);
+    constexpr int O_OB = 2, O_BT = 4;
+    auto cbuf = [&](int b, int j) { return bufs + (size_t)j * C::CBQ + b * C::CB; };
+    auto drain = [&](int j) { return bufs + (size_t)j * C::CBQ; };
     const int tid = threadIdx.x;
     const bool consumer = tid < NC;
     const int ptid = tid - NC;
     const int Ka = g.bra.a.K, Kb = g.bra.single ? 1 : g.bra.b.K;
     const int Kc = g.ket.a.K, Kd = g.ket.single ? 1 : g.ket.b.K;
     const int Kbra = Ka * Kb, Kket = Kc * Kd;
+    const size_t SCRQ = (size_t)Kbra * C::TB + (size_t)Kket * C::TK;      // scratch doubles per quartet
+    double *scr = ga.scratch + (size_t)blockIdx.x * NQ * SCRQ;
 
     // consumer role: chunk ch, quartet slot cj, Hermite rows ip[k]
     int ch = 0, cj = 0, ip[PB], pofs[PB];
@@ -148,6 +181,18 @@ __global__ void __launch_bounds__(MD_F2_PRODUCERS + 192, 1) fused2_kernel(Fused2
             *(long long *)(pq + O_OB) = q * g.s_q + bi * g.s_bi + ki * g.s_ki;
         }
         __syncthreads();
+        // S1 once per group: the 1-D tables of every bra and ket primitive pair of these quartets, by all
+        // threads, into this CTA's scratch (global memory that stays in L2); the producers copy one record per
+        // quartet and batch from there.
+        for (int it = tid; it < 3 * nqg * (Kbra + Kket); it += NT) {
+            const int ax = it % 3, r = it / 3, j = r / (Kbra + Kket), k = r - j * (Kbra + Kket);
+            const int *sidx = (const int *)(perq + (size_t)j * C::PERQ);
+            double *sq = scr + (size_t)j * SCRQ;
+            if (k < Kbra) table_task<LA, LB>(g.bra, sidx[0], sidx[1], k / Kb, k % Kb, ax, sq + (size_t)k * C::TB);
+            else table_task<LC, LD>(g.ket, sidx[2], sidx[3], (k - Kbra) / Kd, (k - Kbra) % Kd, ax,
+                                    sq + (size_t)Kbra * C::TB + (size_t)(k - Kbra) * C::TK);
+        }
+        __syncthreads();
 
         for (int kb = 0; kb < Kbra; ++kb) {
             if (consumer) {
@@ -158,55 +203,52 @@ __global__ void __launch_bounds__(MD_F2_PRODUCERS + 192, 1) fused2_kernel(Fused2
 #pragma unroll
                     for (int i = 0; i < C::NACC; ++i) hacc[k][i] = 0.0;
                 for (int kk = 0; kk < Kket; ++kk) {
-                    const int buf = kk & 1;
+                    const int buf = (kk & 1) * 2 + (kk >> 1 & 1);          // group kk&1, its slot (kk>>1)&1
                     bar_sync(F2_BAR_FULL + buf, NC + NP / 2);
                     if (cact && cj < nqg) {
-                        const double *rec = batch + ((size_t)buf * NQ + cj) * C::BREC;
-                        const double *Rb = rec + C::O_A;
+                        const double *rec = cbuf(buf, cj);
+                        const double *Rb = rec + C::O_R;
                         const double *EP = rec + C::O_EP;
                         if (NCH == 1 || ch == 0) f2_contract<C, LC, LD, PB, NCH, 0>(hacc, Rb, pofs, EP);
                         if constexpr (NCH > 1) { if (ch == 1) f2_contract<C, LC, LD, PB, NCH, 1>(hacc, Rb, pofs, EP); }
                         if constexpr (NCH > 2) { if (ch == 2) f2_contract<C, LC, LD, PB, NCH, 2>(hacc, Rb, pofs, EP); }
                     }
-                    if (kk + 2 < Kket) bar_arrive(F2_BAR_EMPTY + buf, NC + NP / 2);
+                    if (kk + 4 < Kket) bar_arrive(F2_BAR_EMPTY + buf, NC + NP / 2);
                 }
+                bar_sync(F2_BAR_CONS, NC);                   // every consumer is done with the buffers: they become the drain region
                 if (cact && cj < nqg)
-                    f2_flush<C, LD, PURE, PB>(hacc, ch * C::CHC, ip, perq + (size_t)cj * C::PERQ + O_HALF);
+                    f2_flush<C, LD, PURE, PB>(hacc, ch * C::CHC, ip, drain(cj) + C::O_HALF);
             } else {
                 // ---------------- producers: tables, Boys, Hermite Coulomb tensors ----------------
-                // Two producer groups work on alternate ket primitives (group g fills buffer g), so that
-                // each has two consumer batches of time for its four dependent stages.
-                for (int it = ptid; it < 3 * nqg; it += NP) {             // bra tables of primitive kb
-                    const int j = it / 3, ax = it - 3 * j;
-                    double *pq = perq + (size_t)j * C::PERQ;
-                    const int *sidx = (const int *)pq;
-                    table_task<LA, LB>(g.bra, sidx[0], sidx[1], kb / Kb, kb % Kb, ax, pq + O_BT);
-                }
+                // Two producer groups work on alternate ket primitives, each with two buffers of its own, so
+                // that a group has two consumer batches of time for its four dependent stages.
+                for (int j = 0; j < nqg; ++j)                             // bra table records of primitive kb
+                    copy_in(perq + (size_t)j * C::PERQ + O_BT, scr + (size_t)j * SCRQ + (size_t)kb * C::TB, C::TB, ptid, NP);
                 bar_sync(F2_BAR_PALL, NP);
                 const int NG = NP / 2, pgp = ptid / NG, gt = ptid - pgp * NG;
-                double *brec = batch + (size_t)pgp * NQ * C::BREC;
+                double *gs0 = gsc + (size_t)pgp * NQ * C::GS;
                 for (int kk = pgp; kk < Kket; kk += 2) {
-                    if (kk >= 2) bar_sync(F2_BAR_EMPTY + pgp, NC + NG);
-                    for (int it = gt; it < 3 * nqg; it += NG) {           // stage 0: ket tables of primitive kk
-                        const int j = it / 3, ax = it - 3 * j;
-                        const int *sidx = (const int *)(perq + (size_t)j * C::PERQ);
-                        table_task<LC, LD>(g.ket, sidx[2], sidx[3], kk / Kd, kk % Kd, ax, brec + (size_t)j * C::BREC + C::O_TK);
+                    const int buf = pgp * 2 + (kk >> 1 & 1);
+                    if (kk >= 4) bar_sync(F2_BAR_EMPTY + buf, NC + NG);
+                    {                                                     // stage 0: ket table records of primitive kk
+                        const int tpq = NG / nqg, j = gt / tpq;           // a few threads per quartet, no division in the loop
+                        if (j < nqg)
+                            copy_in(gs0 + (size_t)j * C::GS + C::O_TK,
+                                    scr + (size_t)j * SCRQ + (size_t)Kbra * C::TB + (size_t)kk * C::TK, C::TK, gt - j * tpq, tpq);
                     }
                     bar_sync(F2_BAR_PROD + pgp, NG);
                     if (gt < nqg) {                                       // stage 1a: Boys, [0]^(m), z-line
-                        I::z_task(perq + (size_t)gt * C::PERQ + O_BT, brec + (size_t)gt * C::BREC, g.boys_tab);
+                        I::z_task(perq + (size_t)gt * C::PERQ + O_BT, gs0 + (size_t)gt * C::GS, cbuf(buf, gt), g.boys_tab);
                     } else if (gt >= NQ) {                                // stage 1b: ket products, q~-major
                         const int nw = NG - NQ, w = gt - NQ;
                         for (int j = 0; j < nqg; ++j) {
-                            double *rec = brec + (size_t)j * C::BREC;
-#pragma unroll 4
-                            for (int e = w; e < C::EPK; e += nw) rec[C::O_EP + e] = prod_entry(rec + C::O_TK, packq[e]);
+                            prod_list(gs0 + (size_t)j * C::GS + C::O_TK, packq, cbuf(buf, j) + C::O_EP, C::EPK, w, nw);
                         }
                     }
                     bar_sync(F2_BAR_PROD + pgp, NG);
                     for (int it = gt; it < (L + 1) * nqg; it += NG) {     // stage y (tasks sorted by line length)
                         const int v = it / nqg, j = it - v * nqg;
-                        I::y_task(v, brec + (size_t)j * C::BREC);
+                        I::y_task(v, gs0 + (size_t)j * C::GS, cbuf(buf, j));
                     }
                     bar_sync(F2_BAR_PROD + pgp, NG);
                     for (int it = gt; it < C::NZ * nqg; it += NG) {       // stage x (sorted by line length)
@@ -214,23 +256,19 @@ __global__ void __launch_bounds__(MD_F2_PRODUCERS + 192, 1) fused2_kernel(Fused2
                         const int j = it - c * nqg;
                         int s = 0;
                         while (c > s) { c -= s + 1; ++s; }                // column c of the anti-diagonal u+v = s
-                        I::x_task(c, s - c, brec + (size_t)j * C::BREC);
+                        I::x_task(c, s - c, gs0 + (size_t)j * C::GS, cbuf(buf, j));
                     }
-                    bar_arrive(F2_BAR_FULL + pgp, NC + NG);
-                }
-                // bra products of primitive kb (component-major list for P5)
-                for (int j = 0; j < nqg; ++j) {
-                    double *pq = perq + (size_t)j * C::PERQ;
-#pragma unroll 4
-                    for (int e = ptid; e < C::NPB; e += NP) pq[O_EPB + e] = prod_entry(pq + O_BT, packc[e]);
+                    bar_arrive(F2_BAR_FULL + buf, NC + NG);
                 }
             }
-            __syncthreads();                                 // [p~|c md] rows and bra products are in place
+            __syncthreads();                                 // [p~|c md] rows are in place; the buffers are free
+            for (int j = 0; j < nqg; ++j)                    // bra products of primitive kb (component-major list for P5)
+                prod_list(perq + (size_t)j * C::PERQ + O_BT, packc, drain(j) + C::O_EPB, C::NPB, tid, NT);
             if constexpr (PURE && LC > 0) {                  // ket c-index transform, in place per (p~, md)
                 constexpr SolidTab<LC> S{};
                 for (int it = tid; it < nqg * C::NHB * C::NDO; it += NT) {
                     const int j = it / (C::NHB * C::NDO), r = it - j * (C::NHB * C::NDO), p = r / C::NDO, md = r - p * C::NDO;
-                    double *row = perq + (size_t)j * C::PERQ + O_HALF + p * C::HS + md;
+                    double *row = drain(j) + C::O_HALF + p * C::HS + md;
                     double x[C::NCC];
 #pragma unroll
                     for (int c = 0; c < C::NCC; ++c) x[c] = row[c * C::NDO];
@@ -243,20 +281,20 @@ __global__ void __launch_bounds__(MD_F2_PRODUCERS + 192, 1) fused2_kernel(Fused2
                         row[m * C::NDO] = s;
                     }
                 }
-                __syncthreads();
             }
+            __syncthreads();
             // P5: [ab|cd] += sum_p~ E^{ab}_{p~} [p~|cd]  (Eq. 26), bra transform, accumulate in the output
             for (int it = tid; it < nqg * C::NCD_O; it += NT) {
                 const int j = it / C::NCD_O, icd = it - j * C::NCD_O;
                 const double *pq = perq + (size_t)j * C::PERQ;
-                const double *half = pq + O_HALF + icd;
+                const double *half = drain(j) + C::O_HALF + icd;
                 double hv[C::NHB];
 #pragma unroll
                 for (int i = 0; i < C::NHB; ++i) hv[i] = half[i * C::HS];
                 double oacc[C::NAB_C];
 #pragma unroll
                 for (int i = 0; i < C::NAB_C; ++i) oacc[i] = 0.0;
-                const double2 *ep = (const double2 *)(pq + O_EPB);
+                const double2 *ep = (const double2 *)(drain(j) + C::O_EPB);
                 constexpr ProdList<LA, LB, 0> PBL{};
                 double2 e2 = make_double2(0.0, 0.0);
                 static_for<PBL.N>([&](auto ic) {

@@ -177,16 +177,19 @@ struct PMap {
 template <int Lb, int PB, int L>
 __device__ const PMap<Lb, PB, L> d_pmap{};
 
-// One word per product-list position: where its three 1-D factors sit inside a table record
-// (offset 8 + axis*E1 + row + t, 10 bits each), bit 30 = the sign (-1)^{t+u+v} of PAPER.md Eq. 19,
-// bit 31 = valid (padding positions are written as zero).
-__host__ __device__ constexpr unsigned prod_word(int L1, int L2, XYZ a, XYZ b, int t, int u, int v) {
+// One word per product-list position: four byte offsets into a table record (fused2_kernel.cuh),
+//   byte 0 = the coefficient slot (4: +c_a c_b, 5: -c_a c_b for odd t+u+v, the sign of PAPER.md Eq. 19,
+//            6: 0.0 for padding positions), bytes 1-3 = the x, y and z factors (8 + axis*E1 + row + t),
+// so that an entry is the product of four shared-memory loads with no select.
+__host__ __device__ constexpr unsigned prod_word(int L1, int L2, XYZ a, XYZ b, int t, int u, int v, bool sign) {
     const int E1 = e1_count(L1, L2);
     const unsigned ox = 8 + e1_rowoff(L2, a.x, b.x) + t;
     const unsigned oy = 8 + E1 + e1_rowoff(L2, a.y, b.y) + u;
     const unsigned oz = 8 + 2 * E1 + e1_rowoff(L2, a.z, b.z) + v;
-    return ox | oy << 10 | oz << 20 | (unsigned)((t + u + v) & 1) << 30 | 1u << 31;
+    const unsigned oc = (sign && ((t + u + v) & 1)) ? 5 : 4;
+    return oc | ox << 8 | oy << 16 | oz << 24;
 }
+constexpr unsigned PROD_WORD_ZERO = 6u | 6u << 8 | 6u << 16 | 6u << 24;
 // q~-major chunked list (ket side, consumer order of ProdQ).
 template <int L1, int L2, int NCH>
 struct ProdPackQ {
@@ -196,10 +199,10 @@ struct ProdPackQ {
         constexpr ProdQ<L1, L2, NCH> PQ{};
         for (int ch = 0; ch < NCH; ++ch)
             for (int e = PQ.choff[ch]; e < PQ.choff[ch + 1]; ++e) {
-                if (PQ.q_of[e] < 0) { w[e] = 0; continue; }
+                if (PQ.q_of[e] < 0) { w[e] = PROD_WORD_ZERO; continue; }
                 const int cd = (ch * PQ.CHC) * PQ.NC2 + PQ.comp_of[e];
                 XYZ a = cart_exp(L1, cd / PQ.NC2), b = cart_exp(L2, cd % PQ.NC2), h = herm_exp(PQ.q_of[e]);
-                w[e] = prod_word(L1, L2, a, b, h.x, h.y, h.z);
+                w[e] = prod_word(L1, L2, a, b, h.x, h.y, h.z, true);
             }
     }
 };
@@ -217,7 +220,7 @@ struct ProdPackC {
                 XYZ a = cart_exp(L1, c), b = cart_exp(L2, d);
                 for (int t = 0; t <= a.x + b.x; ++t)
                     for (int u = 0; u <= a.y + b.y; ++u)
-                        for (int v = 0; v <= a.z + b.z; ++v) w[i++] = prod_word(L1, L2, a, b, t, u, v) & ~(1u << 30);
+                        for (int v = 0; v <= a.z + b.z; ++v) w[i++] = prod_word(L1, L2, a, b, t, u, v, false);
             }
     }
 };

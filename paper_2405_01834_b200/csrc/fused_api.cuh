@@ -14,9 +14,10 @@ int fused_dispatch(const PairView &b, const PairView &k, long long nq, const int
                    double *out, const double *boys_tab, int nsm, cudaStream_t st, bool force);
 
 // Warp-specialised fused kernels (fused2_inst.cu): same contract as fused_dispatch; info (may be null)
-// receives {PB, NCH, NQ, consumer threads, smem bytes}.
+// receives {PB, NCH, NQ, consumer threads, smem bytes}; get_ws supplies the per-CTA pair-table scratch
+// (returns < 0 with that error code if it cannot).
 cudaError_t fused2_init(int max_smem);
 int fused2_dispatch(const PairView &b, const PairView &k, long long nq, const int32_t *qidx, int pure, int layout,
-                    double *out, const double *boys_tab, int nsm, cudaStream_t st, int *info);
+                    double *out, const double *boys_tab, int nsm, cudaStream_t st, int *info, int (*get_ws)(size_t, void **));
 
 }  // namespace mdb
