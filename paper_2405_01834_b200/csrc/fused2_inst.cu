@@ -10,7 +10,7 @@ namespace {
 
 struct F2Entry {
     void (*fn)(Fused2Args);
-    int pb, nch, npg, tb, tk;
+    int pb, nch, npg, tb, tk, krec;
     size_t perq_bytes, fixed_bytes;   // shared memory per quartet slot and per CTA
 };
 F2Entry g_f2[3 * 3 * 3 * 3 * 2];
@@ -23,7 +23,7 @@ cudaError_t reg(int max_smem) {
     auto fn = fused2_kernel<LA, LB, LC, LD, PURE, PB, NCH>;
     cudaError_t err = cudaFuncSetAttribute(fn, cudaFuncAttributeMaxDynamicSharedMemorySize, max_smem);
     if (err != cudaSuccess) return err;
-    e.fn = fn; e.pb = PB; e.nch = NCH; e.npg = C::NPG; e.tb = C::TB; e.tk = C::TK; e.fixed_bytes = C::smem_bytes(0); e.perq_bytes = C::smem_bytes(1) - e.fixed_bytes;
+    e.fn = fn; e.pb = PB; e.nch = NCH; e.npg = C::NPG; e.tb = C::TB; e.tk = C::TK; e.krec = 8 + even_up(C::EPK); e.fixed_bytes = C::smem_bytes(0); e.perq_bytes = C::smem_bytes(1) - e.fixed_bytes;
     return cudaSuccess;
 }
 
@@ -56,7 +56,7 @@ int fused2_dispatch(const PairView &b0, const PairView &k0, long long nq, const 
     const unsigned grid = (unsigned)std::min<long long>(ngroups, nsm);
     const size_t smem = e.perq_bytes * NQ + e.fixed_bytes;
     const int Kbra = ga.f.bra.a.K * (ga.f.bra.single ? 1 : ga.f.bra.b.K), Kket = ga.f.ket.a.K * (ga.f.ket.single ? 1 : ga.f.ket.b.K);
-    const size_t need = 8 * (size_t)grid * NQ * ((size_t)Kbra * e.tb + (size_t)Kket * e.tk);
+    const size_t need = 8 * (size_t)grid * NQ * ((size_t)Kbra * e.tb + (size_t)Kket * e.krec);
     void *ws = nullptr;
     int werr = get_ws(need, &ws);
     if (werr) return werr;

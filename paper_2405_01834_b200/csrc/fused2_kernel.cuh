@@ -56,11 +56,10 @@ struct F2Cfg {
     // producer-group scratch of one quartet: only live while a batch is being built
     static constexpr int O_B = 0;                              // [0uv]^(m) columns
     static constexpr int O_PQ = O_B + even_up(NHL);            // X, Y, Z, pad
-    static constexpr int O_TK = O_PQ + 4;                      // ket table record
     // strides between quartets are 2 mod 4 doubles: lanes that do the same task for 8 consecutive quartets
     // then fall on 8 distinct 8-byte banks
     static constexpr int pad_bank(int x) { return x + ((2 - x) % 4 + 4) % 4; }
-    static constexpr int GS = pad_bank(O_TK + TK);
+    static constexpr int GS = pad_bank(O_PQ + 4);
     static constexpr int CBQ = pad_bank(NBUF * CB);             // the NBUF buffers of one quartet
     // drain region of one quartet, aliased on its NBUF buffers once every batch of the bra primitive is consumed
     static constexpr int O_HALF = 0, O_EPB = even_up(NHB * HS);
@@ -94,7 +93,7 @@ __device__ __forceinline__ void axis_table_compact(double za, double zb, double 
 }
 
 // Table record of one primitive pair: rec[0] = p, rec[1..3] = P, rec[4] = c_a c_b, rec[5] = -c_a c_b,
-// rec[6] = 0, rec[8 + ax*E1 + ..] = the compact 1-D tables (the slots prod_word addresses).
+// rec[6] = 0, rec[7] = 1/p, rec[8 + ax*E1 + ..] = the compact 1-D tables (the slots prod_word addresses).
 template <int L1, int L2>
 __device__ __forceinline__ void table_task(const PairView &pv, long long i1, long long i2, int k1, int k2, int ax, double *rec) {
     constexpr int E1 = e1_count(L1, L2);
@@ -108,7 +107,7 @@ __device__ __forceinline__ void table_task(const PairView &pv, long long i1, lon
     if (ax == 0) {
         rec[0] = p;
         const double c = __ldg(pv.a.coefs + i1 * K1 + k1) * (pv.single ? 1.0 : __ldg(pv.b.coefs + i2 * K2 + k2));
-        rec[4] = c; rec[5] = -c; rec[6] = 0.0; rec[7] = 0.0;
+        rec[4] = c; rec[5] = -c; rec[6] = 0.0; rec[7] = 1.0 / p;
     }
 }
 
@@ -140,15 +139,42 @@ struct F2Impl {
 
     // ---- producer stages -------------------------------------------------------------------
     // stage 1a: Boys function, [0]^(m) and the z-line for one tensor
-    static __device__ __forceinline__ void z_task(const double *bt, double *gs, double *cb, const double *boys_tab) {
-        const double *kt = gs + C::O_TK;
-        const double p = bt[0], q = kt[0];
-        const double X = bt[1] - kt[1], Y = bt[2] - kt[2], Z = bt[3] - kt[3];
-        const double rho = p * q / (p + q);
+    static __device__ __forceinline__ void z_task(const double *bt, const double *kt, double *gs, double *cb,
+                                                  const double *boys_tab) {
+        const double p = bt[0], q = __ldcg(kt), iq = __ldcg(kt + 7);      // kt: ket header in the L2 scratch
+        const double X = bt[1] - __ldcg(kt + 1), Y = bt[2] - __ldcg(kt + 2), Z = bt[3] - __ldcg(kt + 3);
+        const double rs = rsqrt(p + q);                                    // no FP64 division on this path:
+        const double rho = p * q * rs * rs;                                // rho = pq/(p+q)            (Eq. 23)
+        const double T = rho * (X * X + Y * Y + Z * Z);
+        // Boys function, every order from the Taylor table on its own (boys.cuh, scheme 1): the L+8 table
+        // values are loaded once; the L+1 Horner chains are independent, so the chain is 8 FMAs deep.
         double F[L + 1];
-        boys_eval_t<L>(rho * (X * X + Y * Y + Z * Z), boys_tab, F);
+        if (T < MD_BOYS_TASY) {
+            const int i = __double2int_rn(T * MD_BOYS_ISTEP);
+            const double mh = i * MD_BOYS_STEP - T;
+            const double *row = boys_tab + i * MD_BOYS_MTAB;
+            double r[L + 8];
+#pragma unroll
+            for (int k = 0; k < L + 8; ++k) r[k] = __ldg(row + k);
+#pragma unroll
+            for (int m = 0; m <= L; ++m) {
+                double s = r[m + 7] * (1.0 / 5040.0);
+                s = fma(s, mh, r[m + 6] * (1.0 / 720.0));
+                s = fma(s, mh, r[m + 5] * (1.0 / 120.0));
+                s = fma(s, mh, r[m + 4] * (1.0 / 24.0));
+                s = fma(s, mh, r[m + 3] * (1.0 / 6.0));
+                s = fma(s, mh, r[m + 2] * 0.5);
+                s = fma(s, mh, r[m + 1]);
+                F[m] = fma(s, mh, r[m]);
+            }
+        } else {
+            const double it = 1.0 / T, h = 0.5 * it;
+            double f = 0.88622692545275801365 * sqrt(it);
+#pragma unroll
+            for (int m = 0; m <= L; ++m) { F[m] = f; f *= (2 * m + 1) * h; }
+        }
         double a[2][L + 1];
-        double f = 34.98683665524972497 / (p * q * sqrt(p + q));          // 2 pi^{5/2}   (Eq. 21)
+        double f = 34.98683665524972497 * bt[7] * iq * rs;                // 2 pi^{5/2}/(pq sqrt(p+q))   (Eq. 21)
         const double m2r = -2.0 * rho;
 #pragma unroll
         for (int m = 0; m <= L; ++m) { a[0][m] = F[m] * f; f *= m2r; a[1][m] = 0.0; }

@@ -1,5 +1,7 @@
 // fused2_main.cuh -- the kernel body of the warp-specialised fused kernel (see fused2_kernel.cuh).
 #pragma once
+#include <cuda_pipeline.h>
+
 #include "fused2_kernel.cuh"
 
 namespace mdb {
@@ -138,7 +140,8 @@ __global__ void __launch_bounds__(MD_F2_PRODUCERS + 192, 1) fused2_kernel(Fused2
     const int Ka = g.bra.a.K, Kb = g.bra.single ? 1 : g.bra.b.K;
     const int Kc = g.ket.a.K, Kd = g.ket.single ? 1 : g.ket.b.K;
     const int Kbra = Ka * Kb, Kket = Kc * Kd;
-    const size_t SCRQ = (size_t)Kbra * C::TB + (size_t)Kket * C::TK;      // scratch doubles per quartet
+    constexpr int KREC = 8 + even_up(C::EPK);                             // ket scratch record: header + product list
+    const size_t SCRQ = (size_t)Kbra * C::TB + (size_t)Kket * KREC;       // scratch doubles per quartet
     double *scr = ga.scratch + (size_t)blockIdx.x * NQ * SCRQ;
 
     // consumer role: chunk ch, quartet slot cj, Hermite rows ip[k]
@@ -181,18 +184,36 @@ __global__ void __launch_bounds__(MD_F2_PRODUCERS + 192, 1) fused2_kernel(Fused2
             *(long long *)(pq + O_OB) = q * g.s_q + bi * g.s_bi + ki * g.s_ki;
         }
         __syncthreads();
-        // S1 once per group: the 1-D tables of every bra and ket primitive pair of these quartets, by all
-        // threads, into this CTA's scratch (global memory that stays in L2); the producers copy one record per
-        // quartet and batch from there.
-        for (int it = tid; it < 3 * nqg * (Kbra + Kket); it += NT) {
-            const int ax = it % 3, r = it / 3, j = r / (Kbra + Kket), k = r - j * (Kbra + Kket);
+        // S1 once per group, by all threads, into this CTA's scratch (global memory that stays in L2): the 1-D
+        // table record of every bra primitive pair, and for every ket primitive pair its header and its signed
+        // product list E^{cd}_{q~} (-1)^{|q~|} (Eqs. 7, 19), which does not depend on the bra primitive.  The ket
+        // tables pass through shared memory (the batch buffers are idle here), KC ket primitives at a time.
+        for (int it = tid; it < 3 * nqg * Kbra; it += NT) {
+            const int ax = it % 3, r = it / 3, j = r / Kbra, k = r - j * Kbra;
             const int *sidx = (const int *)(perq + (size_t)j * C::PERQ);
-            double *sq = scr + (size_t)j * SCRQ;
-            if (k < Kbra) table_task<LA, LB>(g.bra, sidx[0], sidx[1], k / Kb, k % Kb, ax, sq + (size_t)k * C::TB);
-            else table_task<LC, LD>(g.ket, sidx[2], sidx[3], (k - Kbra) / Kd, (k - Kbra) % Kd, ax,
-                                    sq + (size_t)Kbra * C::TB + (size_t)(k - Kbra) * C::TK);
+            table_task<LA, LB>(g.bra, sidx[0], sidx[1], k / Kb, k % Kb, ax, scr + (size_t)j * SCRQ + (size_t)k * C::TB);
         }
-        __syncthreads();
+        {
+            const int KC = min(Kket, C::CBQ / C::TK);
+            for (int kk0 = 0; kk0 < Kket; kk0 += KC) {
+                const int kc = min(KC, Kket - kk0);
+                for (int it = tid; it < 3 * nqg * kc; it += NT) {
+                    const int ax = it % 3, r = it / 3, j = r / kc, k = r - j * kc;
+                    const int *sidx = (const int *)(perq + (size_t)j * C::PERQ);
+                    table_task<LC, LD>(g.ket, sidx[2], sidx[3], (kk0 + k) / Kd, (kk0 + k) % Kd, ax,
+                                       bufs + (size_t)j * C::CBQ + (size_t)k * C::TK);
+                }
+                __syncthreads();
+                for (int r = tid >> 5; r < nqg * kc; r += NT >> 5) {      // one warp per (quartet, ket primitive)
+                    const int j = r / kc, k = r - j * kc;
+                    const double *tab = bufs + (size_t)j * C::CBQ + (size_t)k * C::TK;
+                    double *rec = scr + (size_t)j * SCRQ + (size_t)Kbra * C::TB + (size_t)(kk0 + k) * KREC;
+                    if ((tid & 31) < 8) rec[tid & 31] = tab[tid & 31];
+                    prod_list(tab, packq, rec + 8, even_up(C::EPK), tid & 31, 32);
+                }
+                __syncthreads();
+            }
+        }
 
         for (int kb = 0; kb < Kbra; ++kb) {
             if (consumer) {
@@ -230,21 +251,18 @@ __global__ void __launch_bounds__(MD_F2_PRODUCERS + 192, 1) fused2_kernel(Fused2
                 for (int kk = pgp; kk < Kket; kk += 2) {
                     const int buf = pgp * 2 + (kk >> 1 & 1);
                     if (kk >= 4) bar_sync(F2_BAR_EMPTY + buf, NC + NG);
-                    {                                                     // stage 0: ket table records of primitive kk
-                        const int tpq = NG / nqg, j = gt / tpq;           // a few threads per quartet, no division in the loop
-                        if (j < nqg)
-                            copy_in(gs0 + (size_t)j * C::GS + C::O_TK,
-                                    scr + (size_t)j * SCRQ + (size_t)Kbra * C::TB + (size_t)kk * C::TK, C::TK, gt - j * tpq, tpq);
+                    // stage 0: the product lists of ket primitive kk, L2 -> shared memory by asynchronous 16-byte
+                    // copies that complete behind the recursion stages
+                    for (int c = gt; c < nqg * (even_up(C::EPK) / 2); c += NG) {
+                        const int j = c / (even_up(C::EPK) / 2), i = c - j * (even_up(C::EPK) / 2);
+                        __pipeline_memcpy_async(cbuf(buf, j) + C::O_EP + 2 * i,
+                                                scr + (size_t)j * SCRQ + (size_t)Kbra * C::TB + (size_t)kk * KREC + 8 + 2 * i, 16);
                     }
-                    bar_sync(F2_BAR_PROD + pgp, NG);
-                    if (gt < nqg) {                                       // stage 1a: Boys, [0]^(m), z-line
-                        I::z_task(perq + (size_t)gt * C::PERQ + O_BT, gs0 + (size_t)gt * C::GS, cbuf(buf, gt), g.boys_tab);
-                    } else if (gt >= NQ) {                                // stage 1b: ket products, q~-major
-                        const int nw = NG - NQ, w = gt - NQ;
-                        for (int j = 0; j < nqg; ++j) {
-                            prod_list(gs0 + (size_t)j * C::GS + C::O_TK, packq, cbuf(buf, j) + C::O_EP, C::EPK, w, nw);
-                        }
-                    }
+                    __pipeline_commit();
+                    if (gt < nqg)                                         // stage 1: Boys, [0]^(m), z-line
+                        I::z_task(perq + (size_t)gt * C::PERQ + O_BT,
+                                  scr + (size_t)gt * SCRQ + (size_t)Kbra * C::TB + (size_t)kk * KREC, gs0 + (size_t)gt * C::GS,
+                                  cbuf(buf, gt), g.boys_tab);
                     bar_sync(F2_BAR_PROD + pgp, NG);
                     for (int it = gt; it < (L + 1) * nqg; it += NG) {     // stage y (tasks sorted by line length)
                         const int v = it / nqg, j = it - v * nqg;
@@ -258,6 +276,7 @@ __global__ void __launch_bounds__(MD_F2_PRODUCERS + 192, 1) fused2_kernel(Fused2
                         while (c > s) { c -= s + 1; ++s; }                // column c of the anti-diagonal u+v = s
                         I::x_task(c, s - c, gs0 + (size_t)j * C::GS, cbuf(buf, j));
                     }
+                    __pipeline_wait_prior(0);
                     bar_arrive(F2_BAR_FULL + buf, NC + NG);
                 }
             }
