@@ -23,7 +23,7 @@ cudaError_t reg(int max_smem) {
     auto fn = fused2_kernel<LA, LB, LC, LD, PURE, PB, NCH>;
     cudaError_t err = cudaFuncSetAttribute(fn, cudaFuncAttributeMaxDynamicSharedMemorySize, max_smem);
     if (err != cudaSuccess) return err;
-    e.fn = fn; e.pb = PB; e.nch = NCH; e.npg = C::NPG; e.tb = C::TB; e.tk = C::TK; e.krec = 8 + even_up(C::EPK); e.fixed_bytes = C::smem_bytes(0); e.perq_bytes = C::smem_bytes(1) - e.fixed_bytes;
+    e.fn = fn; e.pb = PB; e.nch = NCH; e.npg = C::NPG; e.tb = C::TB; e.tk = C::TK; e.krec = 8 + even_up(C::EPK); e.tb = 8 + even_up(C::NPB); e.fixed_bytes = C::smem_bytes(0); e.perq_bytes = C::smem_bytes(1) - e.fixed_bytes;
     return cudaSuccess;
 }
 

@@ -63,9 +63,10 @@ struct F2Cfg {
     static constexpr int CBQ = pad_bank(NBUF * CB);             // the NBUF buffers of one quartet
     // drain region of one quartet, aliased on its NBUF buffers once every batch of the bra primitive is consumed
     static constexpr int O_HALF = 0, O_EPB = even_up(NHB * HS);
-    static_assert(O_EPB + even_up(NPB) <= NBUF * CB, "drain region must fit in the batch buffers");
-    // per quartet, never aliased: shell indices, output base, bra table record
-    static constexpr int PERQ = 4 + TB;
+    static_assert(O_EPB <= 2 * CB, "the [p~|c md] rows must fit in the two buffers of one producer group");
+    static constexpr bool EPB_SMEM = O_EPB + even_up(NPB) <= 2 * CB;   // else P5 reads the bra list from the L2 scratch
+    // per quartet, never aliased: shell indices, output base
+    static constexpr int PERQ = 4;
     static constexpr int QTOT = PERQ + CBQ + 2 * GS;
     static constexpr int FIXED = (even_up(EPK) + even_up(NPB)) / 2;    // packed product words (doubles)
     static __host__ __device__ constexpr size_t smem_bytes(int nq) { return 8 * ((size_t)nq * QTOT + FIXED); }
@@ -76,7 +77,7 @@ __device__ __forceinline__ void bar_arrive(int id, int n) {
     __threadfence_block();
     asm volatile("bar.arrive %0, %1;" ::"r"(id), "r"(n) : "memory");
 }
-enum { F2_BAR_PALL = 1, F2_BAR_PROD = 2, F2_BAR_CONS = 4, F2_BAR_FULL = 5, F2_BAR_EMPTY = 9 };   // FULL/EMPTY: 4 ids each
+enum { F2_BAR_PROD = 2, F2_BAR_CONS = 4, F2_BAR_FULL = 5, F2_BAR_EMPTY = 9, F2_BAR_DRAIN = 13 };   // FULL/EMPTY: 4 ids each; PROD, DRAIN: 2
 
 // One axis of the two-centre table, written compactly (rows (i,j), t = 0..i+j).
 template <int L1, int L2>
@@ -141,8 +142,9 @@ struct F2Impl {
     // stage 1a: Boys function, [0]^(m) and the z-line for one tensor
     static __device__ __forceinline__ void z_task(const double *bt, const double *kt, double *gs, double *cb,
                                                   const double *boys_tab) {
-        const double p = bt[0], q = __ldcg(kt), iq = __ldcg(kt + 7);      // kt: ket header in the L2 scratch
-        const double X = bt[1] - __ldcg(kt + 1), Y = bt[2] - __ldcg(kt + 2), Z = bt[3] - __ldcg(kt + 3);
+        // bt, kt: bra and ket primitive-pair headers in the L2 scratch
+        const double p = __ldcg(bt), q = __ldcg(kt), ipq = __ldcg(bt + 7) * __ldcg(kt + 7);
+        const double X = __ldcg(bt + 1) - __ldcg(kt + 1), Y = __ldcg(bt + 2) - __ldcg(kt + 2), Z = __ldcg(bt + 3) - __ldcg(kt + 3);
         const double rs = rsqrt(p + q);                                    // no FP64 division on this path:
         const double rho = p * q * rs * rs;                                // rho = pq/(p+q)            (Eq. 23)
         const double T = rho * (X * X + Y * Y + Z * Z);
@@ -174,7 +176,7 @@ struct F2Impl {
             for (int m = 0; m <= L; ++m) { F[m] = f; f *= (2 * m + 1) * h; }
         }
         double a[2][L + 1];
-        double f = 34.98683665524972497 * bt[7] * iq * rs;                // 2 pi^{5/2}/(pq sqrt(p+q))   (Eq. 21)
+        double f = 34.98683665524972497 * ipq * rs;                       // 2 pi^{5/2}/(pq sqrt(p+q))   (Eq. 21)
         const double m2r = -2.0 * rho;
 #pragma unroll
         for (int m = 0; m <= L; ++m) { a[0][m] = F[m] * f; f *= m2r; a[1][m] = 0.0; }

@@ -123,26 +123,34 @@ __global__ void __launch_bounds__(MD_F2_PRODUCERS + 192, 1) fused2_kernel(Fused2
     constexpr int L = C::L;
     const FusedArgs &g = ga.f;
     extern __shared__ double sm[];
-    const int NQ = ga.NQ, NC = NCH * ga.TCH, NT = blockDim.x, NP = NT - NC;
-    // carve-up: [NQ] x { sidx[4 ints], obase, pad, BT }, [NQ] x NBUF consumer buffers (the drain region
-    // {half, EPB} of a quartet aliases its buffers), 2 x [NQ] producer-group scratch, packed product words
+    const int NQ = ga.NQ, NC = NCH * ga.TCH, NT = blockDim.x, NP = NT - NC, NG = NP / 2;
+    // carve-up: [NQ] x { sidx[4 ints], output base, pad }, [NQ] x NBUF consumer buffers, 2 x [NQ] producer-group
+    // scratch, packed product words.  The drain region {[p~|c md] rows, bra products} of a quartet aliases the
+    // two buffers of the producer group that built the last batch of the bra primitive.
     double *perq = sm;
     double *bufs = sm + (size_t)NQ * C::PERQ;
     double *gsc = bufs + (size_t)NQ * C::CBQ;
     unsigned *packq = (unsigned *)(gsc + (size_t)2 * NQ * C::GS);          // [EPK]  ket product words
     unsigned *packc = packq + even_up(C::EPK);                             // [NPB]  bra product words
-    constexpr int O_OB = 2, O_BT = 4;
+    constexpr int O_OB = 2;
+    constexpr int EPKe = even_up(C::EPK), NPBe = even_up(C::NPB);
+    constexpr int KREC = 8 + EPKe, BRECS = 8 + NPBe;                       // scratch records: header + product list
     auto cbuf = [&](int b, int j) { return bufs + (size_t)j * C::CBQ + b * C::CB; };
-    auto drain = [&](int j) { return bufs + (size_t)j * C::CBQ; };
     const int tid = threadIdx.x;
     const bool consumer = tid < NC;
     const int ptid = tid - NC;
     const int Ka = g.bra.a.K, Kb = g.bra.single ? 1 : g.bra.b.K;
     const int Kc = g.ket.a.K, Kd = g.ket.single ? 1 : g.ket.b.K;
-    const int Kbra = Ka * Kb, Kket = Kc * Kd;
-    constexpr int KREC = 8 + even_up(C::EPK);                             // ket scratch record: header + product list
-    const size_t SCRQ = (size_t)Kbra * C::TB + (size_t)Kket * KREC;       // scratch doubles per quartet
+    const int Kbra = Ka * Kb, Kket = Kc * Kd, B = Kbra * Kket;             // B batches per group of quartets
+    const size_t SCRQ = (size_t)Kbra * BRECS + (size_t)Kket * KREC;        // scratch doubles per quartet
     double *scr = ga.scratch + (size_t)blockIdx.x * NQ * SCRQ;
+    auto scr_bra = [&](int j, int kb) { return scr + (size_t)j * SCRQ + (size_t)kb * BRECS; };
+    auto scr_ket = [&](int j, int kk) { return scr + (size_t)j * SCRQ + (size_t)Kbra * BRECS + (size_t)kk * KREC; };
+    // batch b = kb*Kket + kk is built by producer group b&1 in that group's buffer slot (b>>1)&1
+    auto buf_of = [](int b) { return (b & 1) * 2 + (b >> 1 & 1); };
+    auto is_last = [&](int b) { return b < B && b % Kket == Kket - 1; };   // last batch of its bra primitive
+    // buffers that become a drain region are released by the drain's last barrier, not by the EMPTY handshake
+    auto deferred = [&](int b) { return is_last(b) || is_last(b + 2); };
 
     // consumer role: chunk ch, quartet slot cj, Hermite rows ip[k]
     int ch = 0, cj = 0, ip[PB], pofs[PB];
@@ -161,9 +169,10 @@ __global__ void __launch_bounds__(MD_F2_PRODUCERS + 192, 1) fused2_kernel(Fused2
             pofs[k] = C::BR.A * (w & 0xff) + C::BR.B * (w >> 8 & 0xff) + (w >> 16);
         }
     }
-
     for (int e = tid; e < C::EPK; e += NT) packq[e] = d_packq<LC, LD, NCH>.w[e];
     for (int e = tid; e < C::NPB; e += NT) packc[e] = d_packc<LA, LB>.w[e];
+    if (tid < EPKe - C::EPK) packq[C::EPK + tid] = PROD_WORD_ZERO;
+    if (tid < NPBe - C::NPB) packc[C::NPB + tid] = PROD_WORD_ZERO;
 
     const long long ngroups = (g.nq + NQ - 1) / NQ;
     for (long long grp = blockIdx.x; grp < ngroups; grp += gridDim.x) {
@@ -184,110 +193,52 @@ __global__ void __launch_bounds__(MD_F2_PRODUCERS + 192, 1) fused2_kernel(Fused2
             *(long long *)(pq + O_OB) = q * g.s_q + bi * g.s_bi + ki * g.s_ki;
         }
         __syncthreads();
-        // S1 once per group, by all threads, into this CTA's scratch (global memory that stays in L2): the 1-D
-        // table record of every bra primitive pair, and for every ket primitive pair its header and its signed
-        // product list E^{cd}_{q~} (-1)^{|q~|} (Eqs. 7, 19), which does not depend on the bra primitive.  The ket
-        // tables pass through shared memory (the batch buffers are idle here), KC ket primitives at a time.
-        for (int it = tid; it < 3 * nqg * Kbra; it += NT) {
-            const int ax = it % 3, r = it / 3, j = r / Kbra, k = r - j * Kbra;
-            const int *sidx = (const int *)(perq + (size_t)j * C::PERQ);
-            table_task<LA, LB>(g.bra, sidx[0], sidx[1], k / Kb, k % Kb, ax, scr + (size_t)j * SCRQ + (size_t)k * C::TB);
-        }
-        {
-            const int KC = min(Kket, C::CBQ / C::TK);
-            for (int kk0 = 0; kk0 < Kket; kk0 += KC) {
-                const int kc = min(KC, Kket - kk0);
+        // ---- S1, once per group, by all threads, into this CTA's scratch (global memory that stays in L2): for every
+        // bra and every ket primitive pair of these quartets a record {header, product list}: the 1-D tables
+        // (Eqs. 9, 10, 13, 14) pass through shared memory (the batch buffers are idle here), a chunk of primitives
+        // at a time; the lists E^{ab}_{p~} and E^{cd}_{q~}(-1)^{|q~|} (Eqs. 7, 19) do not depend on the other side.
+        auto build_side = [&](auto side) {
+            constexpr bool KET = decltype(side)::value;
+            constexpr int T = KET ? C::TK : C::TB, LEN = KET ? EPKe : NPBe;
+            const int K = KET ? Kket : Kbra, K2 = KET ? Kd : Kb;
+            const unsigned *pack = KET ? packq : packc;
+            const int KC = min(K, C::CBQ / T);
+            for (int k0 = 0; k0 < K; k0 += KC) {
+                const int kc = min(KC, K - k0);
                 for (int it = tid; it < 3 * nqg * kc; it += NT) {
                     const int ax = it % 3, r = it / 3, j = r / kc, k = r - j * kc;
                     const int *sidx = (const int *)(perq + (size_t)j * C::PERQ);
-                    table_task<LC, LD>(g.ket, sidx[2], sidx[3], (kk0 + k) / Kd, (kk0 + k) % Kd, ax,
-                                       bufs + (size_t)j * C::CBQ + (size_t)k * C::TK);
+                    double *tab = bufs + (size_t)j * C::CBQ + (size_t)k * T;
+                    if constexpr (KET) table_task<LC, LD>(g.ket, sidx[2], sidx[3], (k0 + k) / K2, (k0 + k) % K2, ax, tab);
+                    else table_task<LA, LB>(g.bra, sidx[0], sidx[1], (k0 + k) / K2, (k0 + k) % K2, ax, tab);
                 }
                 __syncthreads();
-                for (int r = tid >> 5; r < nqg * kc; r += NT >> 5) {      // one warp per (quartet, ket primitive)
+                for (int r = tid >> 5; r < nqg * kc; r += NT >> 5) {      // one warp per (quartet, primitive pair)
                     const int j = r / kc, k = r - j * kc;
-                    const double *tab = bufs + (size_t)j * C::CBQ + (size_t)k * C::TK;
-                    double *rec = scr + (size_t)j * SCRQ + (size_t)Kbra * C::TB + (size_t)(kk0 + k) * KREC;
+                    const double *tab = bufs + (size_t)j * C::CBQ + (size_t)k * T;
+                    double *rec = KET ? scr_ket(j, k0 + k) : scr_bra(j, k0 + k);
                     if ((tid & 31) < 8) rec[tid & 31] = tab[tid & 31];
-                    prod_list(tab, packq, rec + 8, even_up(C::EPK), tid & 31, 32);
+                    prod_list(tab, pack, rec + 8, LEN, tid & 31, 32);
                 }
                 __syncthreads();
             }
-        }
+        };
+        build_side(std::false_type{});
+        build_side(std::true_type{});
 
-        for (int kb = 0; kb < Kbra; ++kb) {
-            if (consumer) {
-                // ---------------- consumers: P4 over the ket primitives ----------------
-                double hacc[PB][C::NACC];
-#pragma unroll
-                for (int k = 0; k < PB; ++k)
-#pragma unroll
-                    for (int i = 0; i < C::NACC; ++i) hacc[k][i] = 0.0;
-                for (int kk = 0; kk < Kket; ++kk) {
-                    const int buf = (kk & 1) * 2 + (kk >> 1 & 1);          // group kk&1, its slot (kk>>1)&1
-                    bar_sync(F2_BAR_FULL + buf, NC + NP / 2);
-                    if (cact && cj < nqg) {
-                        const double *rec = cbuf(buf, cj);
-                        const double *Rb = rec + C::O_R;
-                        const double *EP = rec + C::O_EP;
-                        if (NCH == 1 || ch == 0) f2_contract<C, LC, LD, PB, NCH, 0>(hacc, Rb, pofs, EP);
-                        if constexpr (NCH > 1) { if (ch == 1) f2_contract<C, LC, LD, PB, NCH, 1>(hacc, Rb, pofs, EP); }
-                        if constexpr (NCH > 2) { if (ch == 2) f2_contract<C, LC, LD, PB, NCH, 2>(hacc, Rb, pofs, EP); }
-                    }
-                    if (kk + 4 < Kket) bar_arrive(F2_BAR_EMPTY + buf, NC + NP / 2);
-                }
-                bar_sync(F2_BAR_CONS, NC);                   // every consumer is done with the buffers: they become the drain region
-                if (cact && cj < nqg)
-                    f2_flush<C, LD, PURE, PB>(hacc, ch * C::CHC, ip, drain(cj) + C::O_HALF);
-            } else {
-                // ---------------- producers: tables, Boys, Hermite Coulomb tensors ----------------
-                // Two producer groups work on alternate ket primitives, each with two buffers of its own, so
-                // that a group has two consumer batches of time for its four dependent stages.
-                for (int j = 0; j < nqg; ++j)                             // bra table records of primitive kb
-                    copy_in(perq + (size_t)j * C::PERQ + O_BT, scr + (size_t)j * SCRQ + (size_t)kb * C::TB, C::TB, ptid, NP);
-                bar_sync(F2_BAR_PALL, NP);
-                const int NG = NP / 2, pgp = ptid / NG, gt = ptid - pgp * NG;
-                double *gs0 = gsc + (size_t)pgp * NQ * C::GS;
-                for (int kk = pgp; kk < Kket; kk += 2) {
-                    const int buf = pgp * 2 + (kk >> 1 & 1);
-                    if (kk >= 4) bar_sync(F2_BAR_EMPTY + buf, NC + NG);
-                    // stage 0: the product lists of ket primitive kk, L2 -> shared memory by asynchronous 16-byte
-                    // copies that complete behind the recursion stages
-                    for (int c = gt; c < nqg * (even_up(C::EPK) / 2); c += NG) {
-                        const int j = c / (even_up(C::EPK) / 2), i = c - j * (even_up(C::EPK) / 2);
-                        __pipeline_memcpy_async(cbuf(buf, j) + C::O_EP + 2 * i,
-                                                scr + (size_t)j * SCRQ + (size_t)Kbra * C::TB + (size_t)kk * KREC + 8 + 2 * i, 16);
-                    }
-                    __pipeline_commit();
-                    if (gt < nqg)                                         // stage 1: Boys, [0]^(m), z-line
-                        I::z_task(perq + (size_t)gt * C::PERQ + O_BT,
-                                  scr + (size_t)gt * SCRQ + (size_t)Kbra * C::TB + (size_t)kk * KREC, gs0 + (size_t)gt * C::GS,
-                                  cbuf(buf, gt), g.boys_tab);
-                    bar_sync(F2_BAR_PROD + pgp, NG);
-                    for (int it = gt; it < (L + 1) * nqg; it += NG) {     // stage y (tasks sorted by line length)
-                        const int v = it / nqg, j = it - v * nqg;
-                        I::y_task(v, gs0 + (size_t)j * C::GS, cbuf(buf, j));
-                    }
-                    bar_sync(F2_BAR_PROD + pgp, NG);
-                    for (int it = gt; it < C::NZ * nqg; it += NG) {       // stage x (sorted by line length)
-                        int c = it / nqg;
-                        const int j = it - c * nqg;
-                        int s = 0;
-                        while (c > s) { c -= s + 1; ++s; }                // column c of the anti-diagonal u+v = s
-                        I::x_task(c, s - c, gs0 + (size_t)j * C::GS, cbuf(buf, j));
-                    }
-                    __pipeline_wait_prior(0);
-                    bar_arrive(F2_BAR_FULL + buf, NC + NG);
-                }
-            }
-            __syncthreads();                                 // [p~|c md] rows are in place; the buffers are free
-            for (int j = 0; j < nqg; ++j)                    // bra products of primitive kb (component-major list for P5)
-                prod_list(perq + (size_t)j * C::PERQ + O_BT, packc, drain(j) + C::O_EPB, C::NPB, tid, NT);
+        // ---- the drain of bra primitive kb (Eq. 16 on c, Eq. 26, bra transform, output), run by the consumers and the
+        // producer group dg whose two buffers hold the drain region; t = 0..DN-1 numbers the participants.
+        auto drain_phase = [&](int kb, int dg, int t) {
+            const int DN = NC + NG, DB = F2_BAR_DRAIN + dg;
+            auto dreg = [&](int j) { return cbuf(2 * dg, j); };
+            bar_sync(DB, DN);                                // [p~|c md] rows are flushed; both buffers are free
+            if constexpr (C::EPB_SMEM)
+                for (int j = 0; j < nqg; ++j) copy_in(dreg(j) + C::O_EPB, scr_bra(j, kb) + 8, NPBe, t, DN);
             if constexpr (PURE && LC > 0) {                  // ket c-index transform, in place per (p~, md)
                 constexpr SolidTab<LC> S{};
-                for (int it = tid; it < nqg * C::NHB * C::NDO; it += NT) {
+                for (int it = t; it < nqg * C::NHB * C::NDO; it += DN) {
                     const int j = it / (C::NHB * C::NDO), r = it - j * (C::NHB * C::NDO), p = r / C::NDO, md = r - p * C::NDO;
-                    double *row = drain(j) + C::O_HALF + p * C::HS + md;
+                    double *row = dreg(j) + C::O_HALF + p * C::HS + md;
                     double x[C::NCC];
 #pragma unroll
                     for (int c = 0; c < C::NCC; ++c) x[c] = row[c * C::NDO];
@@ -301,19 +252,18 @@ __global__ void __launch_bounds__(MD_F2_PRODUCERS + 192, 1) fused2_kernel(Fused2
                     }
                 }
             }
-            __syncthreads();
-            // P5: [ab|cd] += sum_p~ E^{ab}_{p~} [p~|cd]  (Eq. 26), bra transform, accumulate in the output
-            for (int it = tid; it < nqg * C::NCD_O; it += NT) {
+            bar_sync(DB, DN);
+            // P5: [ab|cd] += sum_p~ E^{ab}_{p~} [p~|cd]  (Eq. 26), bra transform, accumulate in the output (L2)
+            for (int it = t; it < nqg * C::NCD_O; it += DN) {
                 const int j = it / C::NCD_O, icd = it - j * C::NCD_O;
-                const double *pq = perq + (size_t)j * C::PERQ;
-                const double *half = drain(j) + C::O_HALF + icd;
+                const double *half = dreg(j) + C::O_HALF + icd;
                 double hv[C::NHB];
 #pragma unroll
                 for (int i = 0; i < C::NHB; ++i) hv[i] = half[i * C::HS];
                 double oacc[C::NAB_C];
 #pragma unroll
                 for (int i = 0; i < C::NAB_C; ++i) oacc[i] = 0.0;
-                const double2 *ep = (const double2 *)(drain(j) + C::O_EPB);
+                const double2 *ep = (const double2 *)(C::EPB_SMEM ? dreg(j) + C::O_EPB : scr_bra(j, kb) + 8);
                 constexpr ProdList<LA, LB, 0> PBL{};
                 double2 e2 = make_double2(0.0, 0.0);
                 static_for<PBL.N>([&](auto ic) {
@@ -323,20 +273,84 @@ __global__ void __launch_bounds__(MD_F2_PRODUCERS + 192, 1) fused2_kernel(Fused2
                 });
                 double o2[C::NAB_O];
                 solid2<LA, LB, PURE>(oacc, o2);
-                double *o = g.out + *(const long long *)(pq + O_OB) + (icd / C::NDO) * g.sc + (icd % C::NDO) * g.sd;
-                if (kb == 0) {
+                double *o = g.out + *(const long long *)(perq + (size_t)j * C::PERQ + O_OB) + (icd / C::NDO) * g.sc + (icd % C::NDO) * g.sd;
+                if (kb > 0) {                                // all loads first: the compiler cannot prove the elements distinct
+                    double prev[C::NAB_O];
 #pragma unroll
                     for (int a = 0; a < C::NAO; ++a)
 #pragma unroll
-                        for (int b = 0; b < C::NBO; ++b) o[a * g.sa + b * g.sb] = o2[a * C::NBO + b];
-                } else {
+                        for (int b = 0; b < C::NBO; ++b) prev[a * C::NBO + b] = __ldcg(o + a * g.sa + b * g.sb);
 #pragma unroll
-                    for (int a = 0; a < C::NAO; ++a)
-#pragma unroll
-                        for (int b = 0; b < C::NBO; ++b) o[a * g.sa + b * g.sb] += o2[a * C::NBO + b];
+                    for (int i = 0; i < C::NAB_O; ++i) o2[i] += prev[i];
                 }
+#pragma unroll
+                for (int a = 0; a < C::NAO; ++a)
+#pragma unroll
+                    for (int b = 0; b < C::NBO; ++b) o[a * g.sa + b * g.sb] = o2[a * C::NBO + b];
             }
-            __syncthreads();                                 // rows, products and tables may be rewritten
+            bar_sync(DB, DN);                                // the drain region is free again
+        };
+
+        if (consumer) {
+            // ---------------- consumers: P4 over the ket primitives, then the drain ----------------
+            for (int kb = 0; kb < Kbra; ++kb) {
+                double hacc[PB][C::NACC];
+#pragma unroll
+                for (int k = 0; k < PB; ++k)
+#pragma unroll
+                    for (int i = 0; i < C::NACC; ++i) hacc[k][i] = 0.0;
+                for (int kk = 0; kk < Kket; ++kk) {
+                    const int b = kb * Kket + kk, buf = buf_of(b);
+                    bar_sync(F2_BAR_FULL + buf, NC + NG);
+                    if (cact && cj < nqg) {
+                        const double *rec = cbuf(buf, cj);
+                        const double *Rb = rec + C::O_R;
+                        const double *EP = rec + C::O_EP;
+                        if (NCH == 1 || ch == 0) f2_contract<C, LC, LD, PB, NCH, 0>(hacc, Rb, pofs, EP);
+                        if constexpr (NCH > 1) { if (ch == 1) f2_contract<C, LC, LD, PB, NCH, 1>(hacc, Rb, pofs, EP); }
+                        if constexpr (NCH > 2) { if (ch == 2) f2_contract<C, LC, LD, PB, NCH, 2>(hacc, Rb, pofs, EP); }
+                    }
+                    if (b + 4 < B && !deferred(b)) bar_arrive(F2_BAR_EMPTY + buf, NC + NG);
+                }
+                const int dg = (kb * Kket + Kket - 1) & 1;
+                bar_sync(F2_BAR_CONS, NC);                   // every consumer is done with group dg's buffers
+                if (cact && cj < nqg) f2_flush<C, LD, PURE, PB>(hacc, ch * C::CHC, ip, cbuf(2 * dg, cj) + C::O_HALF);
+                drain_phase(kb, dg, tid);
+            }
+        } else {
+            // ---------------- producers: Boys, Hermite Coulomb tensors, product-list streaming ----------------
+            // Two groups build alternate batches, each in two buffers of its own, and run ahead across bra primitives.
+            const int pgp = ptid / NG, gt = ptid - pgp * NG;
+            double *gs0 = gsc + (size_t)pgp * NQ * C::GS;
+            for (int b = pgp; b < B; b += 2) {
+                const int kb = b / Kket, kk = b - kb * Kket, buf = buf_of(b);
+                if (b >= 4 && !deferred(b - 4)) bar_sync(F2_BAR_EMPTY + buf, NC + NG);
+                // stage 0: the product list of ket primitive kk, L2 -> shared memory by asynchronous 16-byte copies
+                // that complete behind the recursion stages
+                for (int c = gt; c < nqg * (EPKe / 2); c += NG) {
+                    const int j = c / (EPKe / 2), i = c - j * (EPKe / 2);
+                    __pipeline_memcpy_async(cbuf(buf, j) + C::O_EP + 2 * i, scr_ket(j, kk) + 8 + 2 * i, 16);
+                }
+                __pipeline_commit();
+                if (gt < nqg)                                             // stage 1: Boys, [0]^(m), z-line
+                    I::z_task(scr_bra(gt, kb), scr_ket(gt, kk), gs0 + (size_t)gt * C::GS, cbuf(buf, gt), g.boys_tab);
+                bar_sync(F2_BAR_PROD + pgp, NG);
+                for (int it = gt; it < (L + 1) * nqg; it += NG) {         // stage y (tasks sorted by line length)
+                    const int v = it / nqg, j = it - v * nqg;
+                    I::y_task(v, gs0 + (size_t)j * C::GS, cbuf(buf, j));
+                }
+                bar_sync(F2_BAR_PROD + pgp, NG);
+                for (int it = gt; it < C::NZ * nqg; it += NG) {           // stage x (sorted by line length)
+                    int c = it / nqg;
+                    const int j = it - c * nqg;
+                    int s = 0;
+                    while (c > s) { c -= s + 1; ++s; }                    // column c of the anti-diagonal u+v = s
+                    I::x_task(c, s - c, gs0 + (size_t)j * C::GS, cbuf(buf, j));
+                }
+                __pipeline_wait_prior(0);
+                bar_arrive(F2_BAR_FULL + buf, NC + NG);
+                if (kk == Kket - 1) drain_phase(kb, pgp, NC + gt);        // this group's buffers become the drain region
+            }
         }
     }
 }
