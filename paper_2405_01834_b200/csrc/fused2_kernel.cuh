@@ -42,7 +42,7 @@ struct F2Cfg {
     static constexpr int TB = even_up(8 + 3 * E1B), TK = even_up(8 + 3 * E1K);   // table records
     static constexpr int NPB = ProdCount<LA, LB>::value();
     static constexpr int EPK = ProdQ<LC, LD, NCH>{}.len();
-    static constexpr int HW = NCC * NDO;                       // [c][md] before the c transform
+    static constexpr int HW = NCO * NDO;                       // cd_out: both ket transforms are applied before the flush
     static constexpr int HS = HW | 1;                          // odd row stride: conflict-free columns
     static constexpr int NZ = (L + 1) * (L + 2) / 2;           // entries of the z-line output
     static constexpr Brick BR = brick_layout(L, Lb);
@@ -63,8 +63,7 @@ struct F2Cfg {
     static constexpr int CBQ = pad_bank(NBUF * CB);             // the NBUF buffers of one quartet
     // drain region of one quartet, aliased on its NBUF buffers once every batch of the bra primitive is consumed
     static constexpr int O_HALF = 0, O_EPB = even_up(NHB * HS);
-    static_assert(O_EPB <= 2 * CB, "the [p~|c md] rows must fit in the two buffers of one producer group");
-    static constexpr bool EPB_SMEM = O_EPB + even_up(NPB) <= 2 * CB;   // else P5 reads the bra list from the L2 scratch
+    static_assert(O_EPB <= 2 * CB, "the [p~|cd] rows must fit in the two buffers of one producer group");
     // per quartet, never aliased: shell indices, output base
     static constexpr int PERQ = 4;
     static constexpr int QTOT = PERQ + CBQ + 2 * GS;

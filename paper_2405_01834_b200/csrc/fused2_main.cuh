@@ -87,31 +87,49 @@ __device__ __forceinline__ void copy_in(double *dst, const double *src, int n, i
     }
 }
 
-// Flush of one chunk: ket d-index transform in registers (Eq. 16), rows to shared memory.
-template <class C, int LD, bool PURE, int PB>
+// Flush of one chunk of a consumer thread's [p~|cd] accumulators to the drain rows half[p~][cd_out].
+// Cartesian output: the chunk's own columns.  Solid output: both ket transforms (Eq. 16) in registers -- the d
+// index fully, the c index over the chunk's components only -- so the row receives a partial sum; chunk 0
+// stores, later chunks add (ADD), in chunk order, with a consumer barrier between the rounds.
+template <class C, int LC, int LD, bool PURE, int PB, bool ADD>
 __device__ __forceinline__ void f2_flush(const double (&hacc)[PB][C::NACC], int c0, const int (&ip)[PB], double *half) {
 #pragma unroll
     for (int k = 0; k < PB; ++k) {
         if (ip[k] < 0) continue;
         double *row = half + ip[k] * C::HS;
+        if constexpr (!PURE) {
 #pragma unroll
-        for (int cl = 0; cl < C::CHC; ++cl) {
-            const int c = c0 + cl;
-            if (c >= C::NCC) break;
-            if constexpr (!PURE) {
+            for (int cl = 0; cl < C::CHC; ++cl) {
+                if (c0 + cl >= C::NCC) break;
 #pragma unroll
-                for (int d = 0; d < C::NCD; ++d) row[c * C::NCD + d] = hacc[k][cl * C::NCD + d];
-            } else {
-                constexpr SolidTab<LD> S{};
+                for (int d = 0; d < C::NCD; ++d) row[(c0 + cl) * C::NCD + d] = hacc[k][cl * C::NCD + d];
+            }
+        } else {
+            constexpr SolidTab<LD> SD{};
+            constexpr SolidTab<LC> SC{};
+            double t[C::CHC][C::NDO];                        // d index transformed
+#pragma unroll
+            for (int cl = 0; cl < C::CHC; ++cl)
 #pragma unroll
                 for (int m = 0; m < C::NDO; ++m) {
                     double s = 0.0;
 #pragma unroll
                     for (int d = 0; d < C::NCD; ++d)
-                        if (S.c[m][d] != 0.0) s = fma(S.c[m][d], hacc[k][cl * C::NCD + d], s);
-                    row[c * C::NDO + m] = s;
+                        if (SD.c[m][d] != 0.0) s = fma(SD.c[m][d], hacc[k][cl * C::NCD + d], s);
+                    t[cl][m] = s;
                 }
-            }
+            // c index: the chunk is known only at run time, the coefficients come from a small constant table
+#pragma unroll
+            for (int mc = 0; mc < C::NCO; ++mc)
+#pragma unroll
+                for (int m = 0; m < C::NDO; ++m) {
+                    double s = ADD ? row[mc * C::NDO + m] : 0.0;
+#pragma unroll
+                    for (int cl = 0; cl < C::CHC; ++cl)
+                        if (c0 + cl < C::NCC) s = fma(d_solidc<LC>.c[mc][c0 + cl], t[cl][m], s);
+                    row[mc * C::NDO + m] = s;
+                }
+            (void)SC;
         }
     }
 }
@@ -231,28 +249,7 @@ __global__ void __launch_bounds__(MD_F2_PRODUCERS + 192, 1) fused2_kernel(Fused2
         auto drain_phase = [&](int kb, int dg, int t) {
             const int DN = NC + NG, DB = F2_BAR_DRAIN + dg;
             auto dreg = [&](int j) { return cbuf(2 * dg, j); };
-            bar_sync(DB, DN);                                // [p~|c md] rows are flushed; both buffers are free
-            if constexpr (C::EPB_SMEM)
-                for (int j = 0; j < nqg; ++j) copy_in(dreg(j) + C::O_EPB, scr_bra(j, kb) + 8, NPBe, t, DN);
-            if constexpr (PURE && LC > 0) {                  // ket c-index transform, in place per (p~, md)
-                constexpr SolidTab<LC> S{};
-                for (int it = t; it < nqg * C::NHB * C::NDO; it += DN) {
-                    const int j = it / (C::NHB * C::NDO), r = it - j * (C::NHB * C::NDO), p = r / C::NDO, md = r - p * C::NDO;
-                    double *row = dreg(j) + C::O_HALF + p * C::HS + md;
-                    double x[C::NCC];
-#pragma unroll
-                    for (int c = 0; c < C::NCC; ++c) x[c] = row[c * C::NDO];
-#pragma unroll
-                    for (int m = 0; m < C::NCO; ++m) {
-                        double s = 0.0;
-#pragma unroll
-                        for (int c = 0; c < C::NCC; ++c)
-                            if (S.c[m][c] != 0.0) s = fma(S.c[m][c], x[c], s);
-                        row[m * C::NDO] = s;
-                    }
-                }
-            }
-            bar_sync(DB, DN);
+            bar_sync(DB, DN);                                // the [p~|cd] rows are flushed
             // P5: [ab|cd] += sum_p~ E^{ab}_{p~} [p~|cd]  (Eq. 26), bra transform, accumulate in the output (L2)
             for (int it = t; it < nqg * C::NCD_O; it += DN) {
                 const int j = it / C::NCD_O, icd = it - j * C::NCD_O;
@@ -263,7 +260,7 @@ __global__ void __launch_bounds__(MD_F2_PRODUCERS + 192, 1) fused2_kernel(Fused2
                 double oacc[C::NAB_C];
 #pragma unroll
                 for (int i = 0; i < C::NAB_C; ++i) oacc[i] = 0.0;
-                const double2 *ep = (const double2 *)(C::EPB_SMEM ? dreg(j) + C::O_EPB : scr_bra(j, kb) + 8);
+                const double2 *ep = (const double2 *)(scr_bra(j, kb) + 8);     // bra product list, L2 scratch through L1
                 constexpr ProdList<LA, LB, 0> PBL{};
                 double2 e2 = make_double2(0.0, 0.0);
                 static_for<PBL.N>([&](auto ic) {
@@ -314,7 +311,19 @@ __global__ void __launch_bounds__(MD_F2_PRODUCERS + 192, 1) fused2_kernel(Fused2
                 }
                 const int dg = (kb * Kket + Kket - 1) & 1;
                 bar_sync(F2_BAR_CONS, NC);                   // every consumer is done with group dg's buffers
-                if (cact && cj < nqg) f2_flush<C, LD, PURE, PB>(hacc, ch * C::CHC, ip, cbuf(2 * dg, cj) + C::O_HALF);
+                if (cact && cj < nqg && ch == 0)
+                    f2_flush<C, LC, LD, PURE, PB, false>(hacc, 0, ip, cbuf(2 * dg, cj) + C::O_HALF);
+                if constexpr (PURE && NCH > 1) {             // solid output: later chunks add their partial c transform
+#pragma unroll
+                    for (int r = 1; r < NCH; ++r) {
+                        bar_sync(F2_BAR_CONS, NC);
+                        if (cact && cj < nqg && ch == r)
+                            f2_flush<C, LC, LD, PURE, PB, true>(hacc, r * C::CHC, ip, cbuf(2 * dg, cj) + C::O_HALF);
+                    }
+                } else if constexpr (NCH > 1) {
+                    if (cact && cj < nqg && ch > 0)
+                        f2_flush<C, LC, LD, PURE, PB, false>(hacc, ch * C::CHC, ip, cbuf(2 * dg, cj) + C::O_HALF);
+                }
                 drain_phase(kb, dg, tid);
             }
         } else {

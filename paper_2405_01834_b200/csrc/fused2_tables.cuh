@@ -253,6 +253,10 @@ struct HermTab {
 template <int N>
 __device__ const HermTab<N> d_herm{};
 
+// Cartesian -> solid coefficients in device memory, for run-time indexed rows/columns.
+template <int L>
+__device__ const SolidTab<L> d_solidc{};
+
 // Cartesian exponents of shell l's components, for lane-varying lookups (x | y<<8 | z<<16).
 template <int L>
 struct CartTab {
