@@ -60,7 +60,7 @@ struct F2Cfg {
     // then fall on 8 distinct 8-byte banks
     static constexpr int pad_bank(int x) { return x + ((2 - x) % 4 + 4) % 4; }
     static constexpr int GS = pad_bank(O_PQ + 4);
-    static constexpr int CBQ = pad_bank(NBUF * CB);             // the NBUF buffers of one quartet
+    static constexpr int CBQ = NBUF * CB + ((10 - NBUF * CB) % 16 + 16) % 16;   // the NBUF buffers of one quartet: 10 (mod 16), see PMap
     // drain region of one quartet, aliased on its NBUF buffers once every batch of the bra primitive is consumed
     static constexpr int O_HALF = 0, O_EPB = even_up(NHB * HS);
     static_assert(O_EPB <= 2 * CB, "the [p~|cd] rows must fit in the two buffers of one producer group");

@@ -183,7 +183,9 @@ __global__ void __launch_bounds__(MD_F2_PRODUCERS + 192, 1) fused2_kernel(Fused2
         for (int k = 0; k < PB; ++k) {
             const int i = d_pmap<C::Lb, PB, L>.p[k][pg];
             ip[k] = cact ? i : -1;
-            const int w = d_herm<C::NHB>.e[i < 0 ? 0 : i];
+            // a lane without a row in this slot reads its neighbour's address (same half-warp: a broadcast)
+            const int in = i < 0 ? d_pmap<C::Lb, PB, L>.p[k][(pg ^ 1) < C::NPG ? (pg ^ 1) : 0] : i;
+            const int w = d_herm<C::NHB>.e[in < 0 ? 0 : in];
             pofs[k] = C::BR.A * (w & 0xff) + C::BR.B * (w >> 8 & 0xff) + (w >> 16);
         }
     }

@@ -127,7 +127,7 @@ __host__ __device__ constexpr Brick brick_layout(int L, int Lb) {
         {5, 0, 16, 22, 111, 1}, {5, 1, 18, 23, 116, 1}, {5, 2, 6, 36, 181, 1},  {5, 3, 18, 23, 116, 2}, {5, 4, 18, 23, 116, 3},
         {6, 0, 22, 28, 169, 1}, {6, 1, 22, 28, 169, 1}, {6, 2, 23, 37, 223, 1}, {6, 3, 22, 35, 211, 2}, {6, 4, 22, 35, 211, 3},
         {7, 0, 29, 37, 260, 1}, {7, 1, 29, 37, 260, 1}, {7, 2, 45, 38, 316, 1}, {7, 3, 40, 29, 281, 2}, {7, 4, 45, 28, 316, 3},
-        {8, 0, 45, 37, 361, 1}, {8, 1, 45, 37, 361, 1}, {8, 2, 60, 35, 481, 1}, {8, 3, 50, 39, 401, 2}, {8, 4, 50, 39, 401, 3}};
+        {8, 0, 45, 37, 361, 1}, {8, 1, 45, 37, 361, 1}, {8, 2, 60, 35, 481, 1}, {8, 3, 50, 39, 401, 2}, {8, 4, 40, 51, 409, 3}};
     for (int i = 0; i < (int)(sizeof(T) / sizeof(T[0])); ++i)
         if (T[i][0] == L && T[i][1] == Lb) return Brick{T[i][2], T[i][3], T[i][4], T[i][5]};
     return Brick{(L + 1) * (L + 1), L + 1, (L + 1) * (L + 1) * (L + 1), 16};      // plain cube
@@ -153,6 +153,17 @@ struct PMap {
     static constexpr int NHB = nherm(Lb), NPG = (NHB + PB - 1) / PB;
     short p[PB][NPG];
     constexpr PMap() : p{} {
+        if (Lb == 4 && PB == 3 && L == 8) {
+            // (dd|dd): rows and lane order found by local search over (A, B, assignment) for the fewest bank
+            // conflicts when a half-warp spans two quartets whose buffers are 10 (mod 16) words apart:
+            // 13 wavefronts over the 9 distinct half-warp patterns (9 would be conflict-free; the greedy rule gives 18).
+            constexpr short T[3][12] = {{10, 0, 18, 28, -1, 19, 21, 7, 26, 24, 16, 30},
+                                        {1, 3, 14, 6, 13, 5, 34, 25, 31, 33, 20, 2},
+                                        {11, 29, 9, 8, 15, 4, 12, 22, 23, 17, 27, 32}};
+            for (int k = 0; k < PB && k < 3; ++k)
+                for (int g = 0; g < NPG && g < 12; ++g) p[k][g] = T[k][g];
+            return;
+        }
         constexpr Brick br = brick_layout(L, Lb);
         int cnt[PB] = {};
         for (int k = 0; k < PB; ++k)
