@@ -59,8 +59,16 @@ __device__ __forceinline__ double prod_entry(const double *tab, unsigned w) {
     return (tab[w & 255] * tab[w >> 8 & 255]) * (tab[w >> 16 & 255] * tab[w >> 24]);
 }
 
-// n products of one table record, entries w, w + stride, ...: all loads of a batch of four entries are
-// issued before the first store (the compiler cannot reorder them itself: same shared array).
+// Store to the per-CTA scratch with an L2 evict_last policy: the scratch is rewritten for every group of
+// quartets and re-read once per bra primitive, so it should stay in L2 and never reach DRAM.
+__device__ __forceinline__ void st_scratch(double *p, double v) {
+    unsigned long long pol;
+    asm volatile("createpolicy.fractional.L2::evict_last.b64 %0, 1.0;" : "=l"(pol));
+    asm volatile("st.global.L2::cache_hint.f64 [%0], %1, %2;" ::"l"(p), "d"(v), "l"(pol) : "memory");
+}
+
+// n products of one table record, entries w, w + stride, ...: written to the scratch; all loads of a
+// batch of four entries are issued before the first store.
 __device__ __forceinline__ void prod_list(const double *tab, const unsigned *pack, double *dst, int n, int w, int stride) {
     for (int e0 = w; e0 < n; e0 += 4 * stride) {
         unsigned ww[4];
@@ -71,7 +79,7 @@ __device__ __forceinline__ void prod_list(const double *tab, const unsigned *pac
         for (int u = 0; u < 4; ++u) v[u] = prod_entry(tab, ww[u]);
 #pragma unroll
         for (int u = 0; u < 4; ++u)
-            if (e0 + u * stride < n) dst[e0 + u * stride] = v[u];
+            if (e0 + u * stride < n) st_scratch(dst + e0 + u * stride, v[u]);
     }
 }
 
@@ -237,7 +245,7 @@ __global__ void __launch_bounds__(MD_F2_PRODUCERS + 192, 1) fused2_kernel(Fused2
                     const int j = r / kc, k = r - j * kc;
                     const double *tab = bufs + (size_t)j * C::CBQ + (size_t)k * T;
                     double *rec = KET ? scr_ket(j, k0 + k) : scr_bra(j, k0 + k);
-                    if ((tid & 31) < 8) rec[tid & 31] = tab[tid & 31];
+                    if ((tid & 31) < 8) st_scratch(rec + (tid & 31), tab[tid & 31]);
                     prod_list(tab, pack, rec + 8, LEN, tid & 31, 32);
                 }
                 __syncthreads();

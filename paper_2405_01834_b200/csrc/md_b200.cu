@@ -228,9 +228,8 @@ int run(const PairView &b, const PairView &k, long long nq, const int32_t *qidx,
     S.last_launches = 0;
     if (nq == 0) return MD_OK;
     if (S.variant == MD_VARIANT_AUTO || S.variant == MD_VARIANT_FUSED2) {
-        // measured faster than the first fused kernel except for uncontracted solid output
-        const long long nprim = (long long)b.a.K * (b.single ? 1 : b.b.K) * k.a.K * (k.single ? 1 : k.b.K);
-        if (S.variant == MD_VARIANT_FUSED2 || nprim > 1 || !pure) {
+        // measured faster than the first fused kernel for every K and both outputs where it is instantiated
+        {
             int r = fused2_dispatch(b, k, nq, qidx, pure, layout, out, S.boys_tab, S.nsm, st, S.last_f2_info, get_workspace);
             if (r == 1) {
                 S.last_launches++;
