@@ -264,6 +264,99 @@ def run_ours(args):
         dist.destroy_process_group()
 
 
+# ------------------------------------------------------------------------------------------------------------
+# Per-class sweep (every class reports its achieved fraction): python bench.py --sweep NAME
+# writes gpurun_out/sweep_NAME.csv; the default run and its one JSON line are unaffected.
+# ------------------------------------------------------------------------------------------------------------
+
+def sweep_cases(name):
+    from paper_2405_01834_b200 import workloads as W
+    cases = []
+    if name == "l2":                 # every class served by both fused kernels, K = 1 and K = 3, solid output
+        pairs = [(1, 1), (2, 0), (2, 1), (2, 2)]
+        for b in pairs:
+            for k in pairs:
+                for K in (1, 3):
+                    n = 100_000 if K == 1 else 20_000
+                    cases.append((f"({b[0]}{b[1]}|{k[0]}{k[1]}) K={K}", lambda b=b, k=k, K=K, n=n: W.independent_quartets(
+                        "sw", b + k, (K,) * 4, n, (0.05, 50.0), (-5.0, 5.0), W.class_seed("l2", b, k, K)), True,
+                        ("fused", "fused2")))
+    elif name == "configs":          # the BASELINE.json configs that exist as generators, AUTO variant
+        cases.append(("cfg1 (pp|pp) K=1 cart n=2000", lambda: W.config1(2000), False, ("auto",)))
+        cases.append(("cfg1-shape (pp|pp) K=1 cart n=1e6", lambda: W.independent_quartets(
+            "sw", (1, 1, 1, 1), (1,) * 4, 1_000_000, (0.1, 20.0), (-3.0, 3.0), 0), False, ("auto",)))
+        for K in (1, 3):
+            for pure in (True, False):
+                cases.append((f"cfg2 (dd|dd) K={K} {'solid' if pure else 'cart'}", lambda K=K: W.config2(K=K), pure, ("auto",)))
+        for (la, lb, lX) in [(0, 0, 0), (1, 1, 1), (2, 2, 2), (3, 3, 3), (3, 3, 6), (2, 1, 4)]:
+            for K in (1, 4):
+                cases.append((f"cfg3 ({la}{lb}|{lX}) K={K} solid", lambda la=la, lb=lb, lX=lX, K=K: W.config3(
+                    la, lb, lX, K=K, n=200_000), True, ("auto",)))
+        for ls in [(3, 3, 3, 3), (4, 4, 4, 4), (5, 5, 5, 5), (6, 6, 6, 6), (3, 4, 5, 6)]:
+            cases.append((f"cfg4 ({ls[0]}{ls[1]}|{ls[2]}{ls[3]}) K=1 solid", lambda ls=ls: W.config4(ls, n=20_000), True, ("auto",)))
+    else:
+        raise SystemExit(f"unknown sweep {name!r}")
+    return cases
+
+
+def run_sweep(args):
+    import numpy as np
+    import torch
+    from paper_2405_01834_b200 import build, engine, workloads as W
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py needs a CUDA device: the engine has no CPU fallback")
+    build.build()
+    torch.cuda.set_device(0)
+    engine.md_init()
+    flush = torch.empty(256 << 20, dtype=torch.uint8, device="cuda")
+    vid = {"auto": engine.VARIANT_AUTO, "generic": engine.VARIANT_GENERIC, "fused": engine.VARIANT_FUSED,
+           "mma": engine.VARIANT_MMA, "fused2": engine.VARIANT_FUSED2}
+    vname = {1: "generic", 2: "fused", 3: "mma", 4: "fused2"}
+    try:
+        hbm = json.load(open(os.path.join(ROOT, "MEASURED_PEAKS.json"))).get("hbm_gbs", 6550.0)
+    except (OSError, ValueError):
+        hbm = 6650.0
+    os.makedirs(os.path.join(ROOT, "gpurun_out"), exist_ok=True)
+    path = os.path.join(ROOT, "gpurun_out", f"sweep_{args.sweep}.csv")
+    rows = ["case,n,variant_asked,variant_used,launches,ms,quartets_per_s,model_flop_per_quartet,model_tflops,"
+            "frac_fp64_peak,out_gbs,frac_hbm"]
+    for label, make, pure, variants in sweep_cases(args.sweep):
+        w = make()
+        for v in variants:
+            engine.md_set_variant(vid[v])
+            try:
+                ww = w
+                if w.nquartets > 2000:                     # bound the time per case: probe on 1000 quartets first
+                    sel = np.arange(1000)
+                    probe = W.Workload("probe", w.a.take(w.shell_indices(sel)[0]), w.b.take(w.shell_indices(sel)[1]),
+                                       w.c.take(w.shell_indices(sel)[2]),
+                                       None if w.three_center else w.d.take(w.shell_indices(sel)[3]), None, None,
+                                       np.stack([np.arange(1000, dtype=np.int32)] * 2, 1))
+                    dp = engine.DeviceWorkload(probe); op = dp.alloc_out(pure)
+                    ms_p = time_steps(lambda: dp.run(pure, op), 2, 2, flush, lambda: None) / 2
+                    cap = int(max(2000, min(w.nquartets, 1000 * 400.0 / max(ms_p, 1e-3))))   # about 0.4 s per step
+                    if cap < w.nquartets:
+                        sel = np.arange(cap)
+                        ia, ib, ic, id_ = w.shell_indices(sel)
+                        ww = W.Workload(w.name, w.a.take(ia), w.b.take(ib), w.c.take(ic),
+                                        None if w.three_center else w.d.take(id_), None, None,
+                                        np.stack([np.arange(cap, dtype=np.int32)] * 2, 1))
+                dw = engine.DeviceWorkload(ww); out = dw.alloc_out(pure)
+                ms = time_steps(lambda: dw.run(pure, out), args.steps, args.warmup, flush, lambda: None) / args.steps
+                used, nl = engine.md_last_variant(), engine.md_last_launch_count()
+                fl = ww.flops_model(pure)
+                tf = fl * ww.nquartets / (ms * 1e-3) / 1e12
+                gbs = out.numel() * 8 / (ms * 1e-3) / 1e9
+                rows.append(f"{label},{ww.nquartets},{v},{vname.get(used, used)},{nl},{ms:.4f},{ww.nquartets / (ms * 1e-3):.4e},"
+                            f"{fl},{tf:.3f},{tf / FP64_PEAK_DERIVED_TFLOPS:.4f},{gbs:.1f},{gbs / hbm:.4f}")
+                print(rows[-1], flush=True)
+                del dw, out
+            finally:
+                engine.md_set_variant(engine.VARIANT_AUTO)
+    open(path, "w").write("\n".join(rows) + "\n")
+    print(json.dumps({"sweep": args.sweep, "csv": os.path.relpath(path, ROOT), "cases": len(rows) - 1}))
+
+
 def main():
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
@@ -272,9 +365,12 @@ def main():
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--variants", action="store_true", help="also time K=1 and Cartesian output")
     ap.add_argument("--cpu-sample", type=int, default=8000)
+    ap.add_argument("--sweep", default=None, help="per-class table instead of the headline: l2 | configs")
     args = ap.parse_args()
     args.warmup = max(args.warmup, 3) if args.impl == "ours" else args.warmup
-    if args.impl == "reference":
+    if args.sweep:
+        run_sweep(args)
+    elif args.impl == "reference":
         run_reference(args)
     else:
         run_ours(args)

@@ -228,8 +228,11 @@ int run(const PairView &b, const PairView &k, long long nq, const int32_t *qidx,
     S.last_launches = 0;
     if (nq == 0) return MD_OK;
     if (S.variant == MD_VARIANT_AUTO || S.variant == MD_VARIANT_FUSED2) {
-        // measured faster than the first fused kernel for every K and both outputs where it is instantiated
-        {
+        // By measurement (profiles/r01_sweep_l2.md): the warp-specialised kernel wins on every instantiated class
+        // once the primitive loop is long enough to fill its pipeline, and on (dd|dd) for any K.
+        const long long nprim = (long long)b.a.K * (b.single ? 1 : b.b.K) * k.a.K * (k.single ? 1 : k.b.K);
+        const bool dddd = b.a.l == 2 && !b.single && b.b.l == 2 && k.a.l == 2 && !k.single && k.b.l == 2;
+        if (S.variant == MD_VARIANT_FUSED2 || nprim >= 4 || (dddd && nq >= 150000)) {
             int r = fused2_dispatch(b, k, nq, qidx, pure, layout, out, S.boys_tab, S.nsm, st, S.last_f2_info, get_workspace);
             if (r == 1) {
                 S.last_launches++;
