@@ -1,6 +1,7 @@
 // host_api.inl -- md_eri4_host / md_eri3_host: the same kernels behind host buffers.
 // Inputs are staged with cudaMemcpyAsync on the caller's stream into stream-ordered
-// temporaries (cudaMallocAsync), the result is copied back, and the stream is synchronised.
+// temporaries (cudaMallocAsync), the result is copied back (overlapped with compute for large quartet
+// lists), and the stream is synchronised.
 namespace {
 
 struct DeviceCopy {
@@ -59,10 +60,35 @@ int host_call(const md_pairs *bra, const md_pairs *ket, const md_shells *X, int6
     if (idx) CK(dc.up(idx, (size_t)n * 2, &didx));
     void *dout = nullptr;
     CK(dc.alloc(&dout, (size_t)need * 8));
-    e = ket ? md_eri4(&dbra, &dket, n, didx, pure, layout, (double *)dout, need, stream)
-            : md_eri3(&dbra, &dX, n, didx, pure, layout, (double *)dout, need, stream);
-    if (e) { cudaStreamSynchronize(st); return e; }
-    CK(cudaMemcpyAsync(out, dout, (size_t)need * 8, cudaMemcpyDeviceToHost, st));
+    // Quartet lists in the quartet-major layout are cut into chunks: the device-to-host copy of chunk i runs on an
+    // internal copy stream while the kernels of chunk i+1 run on the caller's stream.
+    const int64_t per = n > 0 ? need / n : 0;
+    const int nchunk = (idx && layout == MD_LAYOUT_QUARTET_MAJOR && n >= 32768) ? (int)std::min<int64_t>(8, n / 16384) : 1;
+    if (nchunk <= 1) {
+        e = ket ? md_eri4(&dbra, &dket, n, didx, pure, layout, (double *)dout, need, stream)
+                : md_eri3(&dbra, &dX, n, didx, pure, layout, (double *)dout, need, stream);
+        if (e) { cudaStreamSynchronize(st); return e; }
+        CK(cudaMemcpyAsync(out, dout, (size_t)need * 8, cudaMemcpyDeviceToHost, st));
+        CK(cudaStreamSynchronize(st));
+        return MD_OK;
+    }
+    static cudaStream_t copy_stream = nullptr;
+    static cudaEvent_t done[8];
+    if (!copy_stream) {
+        CK(cudaStreamCreateWithFlags(&copy_stream, cudaStreamNonBlocking));
+        for (auto &ev : done) CK(cudaEventCreateWithFlags(&ev, cudaEventDisableTiming));
+    }
+    for (int c = 0; c < nchunk; ++c) {
+        const int64_t q0 = n * c / nchunk, q1 = n * (c + 1) / nchunk, nc = q1 - q0;
+        double *dchunk = (double *)dout + q0 * per;
+        e = ket ? md_eri4(&dbra, &dket, nc, didx + 2 * q0, pure, layout, dchunk, nc * per, stream)
+                : md_eri3(&dbra, &dX, nc, didx + 2 * q0, pure, layout, dchunk, nc * per, stream);
+        if (e) { cudaStreamSynchronize(st); cudaStreamSynchronize(copy_stream); return e; }
+        CK(cudaEventRecord(done[c], st));
+        CK(cudaStreamWaitEvent(copy_stream, done[c], 0));
+        CK(cudaMemcpyAsync(out + q0 * per, dchunk, (size_t)(nc * per) * 8, cudaMemcpyDeviceToHost, copy_stream));
+    }
+    CK(cudaStreamSynchronize(copy_stream));
     CK(cudaStreamSynchronize(st));
     return MD_OK;
 }

@@ -277,6 +277,17 @@ def test_host_buffer_call_matches_device_call():
         assert np.array_equal(host.numpy(), gpu)
 
 
+def test_host_buffer_call_chunked_overlap():
+    """Large quartet lists go through the chunked host call (copy-back overlapped with compute): same bits."""
+    import torch
+    for w, pure in [(W.class_sweep((1, 1, 1, 1), 70001), False), (W.config2(K=2, n=33000), True)]:
+        gpu, _ = gpu_run(w, pure)
+        host = torch.empty(w.nquartets * w.nout(pure), dtype=torch.float64).pin_memory()
+        engine.run_host(w, pure, host)
+        assert np.array_equal(host.numpy(), gpu)
+    check(W.class_sweep((1, 1, 1, 1), 70001), False, sel=np.arange(0, 70001, 997))
+
+
 def test_noncurrent_stream_is_asynchronous_and_correct():
     import torch
     w = W.class_sweep((2, 2, 1, 1), 500)
