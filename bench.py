@@ -299,7 +299,84 @@ def sweep_cases(name):
     return cases
 
 
+def schwarz_factors(engine, W, mol, ta, tb, pairs):
+    """Q_ij = sqrt(max_ab |(ab|ab)|) for every pair of one pair type, with the engine in (i,i) quartet mode."""
+    import numpy as np
+    import torch
+    n = len(pairs)
+    nab = W.nsolid(ta[0]) * W.nsolid(tb[0])
+    q = np.empty(n)
+    step = max(1, (256 << 20) // (8 * nab * nab))
+    for lo in range(0, n, step):
+        hi = min(n, lo + step)
+        ii = np.arange(hi - lo, dtype=np.int32)
+        w = W.config5_class(mol, (ta, tb), (ta, tb), pairs[lo:hi], pairs[lo:hi], np.stack([ii, ii], 1))
+        out = engine.DeviceWorkload(w).run(True).view(hi - lo, nab, nab)
+        q[lo:hi] = torch.sqrt(torch.diagonal(out, dim1=1, dim2=2).abs().amax(dim=1)).cpu().numpy()
+    return q
+
+
+def run_config5(args):
+    """BASELINE configs[4]: the synthetic quadruple-zeta molecule.  Schwarz factors with the engine, exact per-class
+    counts of surviving quartets, every l <= 4 class timed on a seeded sample, sweep time extrapolated."""
+    import numpy as np
+    import torch
+    from paper_2405_01834_b200 import build, engine, workloads as W
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py needs a CUDA device: the engine has no CPU fallback")
+    build.build()
+    torch.cuda.set_device(0)
+    engine.md_init()
+    flush = torch.empty(256 << 20, dtype=torch.uint8, device="cuda")
+    thr = 1e-12
+    mol = W.config5_molecule()
+    ptypes = mol.pair_types(4)
+    pairs = {pt: mol.pair_list(*pt) for pt in ptypes}
+    t0 = time.perf_counter()
+    Q = {pt: schwarz_factors(engine, W, mol, pt[0], pt[1], pairs[pt]) for pt in ptypes}
+    torch.cuda.synchronize()
+    t_schwarz = time.perf_counter() - t0
+    vname = {1: "generic", 2: "fused", 3: "mma", 4: "fused2"}
+    rows = ["class,Kbra,Kket,pairs_bra,pairs_ket,quartets_passing,sampled,variant,ms,quartets_per_s,model_tflops,"
+            "extrapolated_s"]
+    rng = np.random.default_rng(5)
+    tot_q, tot_s, tot_flop = 0, 0.0, 0.0
+    name = lambda t: "spdfg"[t[0]] + (str(t[1]) if t[1] > 1 else "")
+    for ib, pb in enumerate(ptypes):
+        for pk in ptypes[: ib + 1]:
+            same = pb == pk
+            count = W.schwarz_count(Q[pb], Q[pk], thr, same)
+            if count == 0:
+                continue
+            probe = W.schwarz_sample(rng, Q[pb], Q[pk], thr, min(count, 2000), same)
+            wp = W.config5_class(mol, pb, pk, pairs[pb], pairs[pk], probe)
+            dp = engine.DeviceWorkload(wp); op = dp.alloc_out(True)
+            ms_p = time_steps(lambda: dp.run(True, op), 1, 1, flush, lambda: None)
+            n = int(min(count, 200_000, max(len(probe), len(probe) * 100.0 / max(ms_p, 1e-3))))   # about 0.1 s
+            qs = probe if n <= len(probe) else W.schwarz_sample(rng, Q[pb], Q[pk], thr, n, same)
+            w = W.config5_class(mol, pb, pk, pairs[pb], pairs[pk], qs)
+            dw = engine.DeviceWorkload(w); out = dw.alloc_out(True)
+            ms = time_steps(lambda: dw.run(True, out), 2, 1, flush, lambda: None) / 2
+            rate = len(qs) / (ms * 1e-3)
+            fl = w.flops_model(True)
+            cls = f"({name(pb[0])}{name(pb[1])}|{name(pk[0])}{name(pk[1])})"
+            rows.append(f"{cls},{pb[0][1] * pb[1][1]},{pk[0][1] * pk[1][1]},{len(pairs[pb])},{len(pairs[pk])},{count},{len(qs)},"
+                        f"{vname.get(engine.md_last_variant(), '?')},{ms:.4f},{rate:.4e},{fl * rate / 1e12:.3f},{count / rate:.3f}")
+            tot_q += count; tot_s += count / rate; tot_flop += fl * count
+            del dw, out, dp, op
+    path = os.path.join(ROOT, "gpurun_out", "sweep_config5.csv")
+    os.makedirs(os.path.dirname(path), exist_ok=True)
+    open(path, "w").write("\n".join(rows) + "\n")
+    print(json.dumps({"sweep": "config5", "csv": os.path.relpath(path, ROOT), "classes": len(rows) - 1, "shells": mol.nshells(),
+                      "ao_solid": mol.nao(True), "shell_pairs": int(sum(len(p) for p in pairs.values())),
+                      "schwarz_threshold": thr, "schwarz_seconds": t_schwarz, "quartets_passing": tot_q,
+                      "extrapolated_sweep_seconds": tot_s, "extrapolated_model_tflops": tot_flop / tot_s / 1e12,
+                      "note": "per-class rate measured on a seeded sample of the surviving quartets; counts are exact"}))
+
+
 def run_sweep(args):
+    if args.sweep == "config5":
+        return run_config5(args)
     import numpy as np
     import torch
     from paper_2405_01834_b200 import build, engine, workloads as W
@@ -365,7 +442,7 @@ def main():
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--variants", action="store_true", help="also time K=1 and Cartesian output")
     ap.add_argument("--cpu-sample", type=int, default=8000)
-    ap.add_argument("--sweep", default=None, help="per-class table instead of the headline: l2 | configs")
+    ap.add_argument("--sweep", default=None, help="per-class table instead of the headline: l2 | configs | config5")
     args = ap.parse_args()
     args.warmup = max(args.warmup, 3) if args.impl == "ours" else args.warmup
     if args.sweep:

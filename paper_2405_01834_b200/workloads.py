@@ -256,3 +256,106 @@ def paper_microbench(ls, Kbra, Kket, nbra, nket, seed=None, three_center=False):
     seed = class_seed("paper", tuple(ls), Kbra, Kket) if seed is None else seed
     return product_batch("paper_" + "".join(map(str, ls)) + f"_K{Kbra}_{Kket}", ls, Ks, nbra, nket, (0.3, 10.0),
                          (-4.0, 4.0), seed, three_center=three_center)
+
+
+# ---------------------------------------------------------------------------------------
+# BASELINE config 5: synthetic quadruple-zeta-shaped molecule (readings S10, S11)
+# ---------------------------------------------------------------------------------------
+
+# (l, K) of the shells each atom carries, in the order BASELINE.json lists them
+HEAVY_SHELLS = [(0, 6), (0, 1), (0, 1), (0, 1), (1, 3), (1, 1), (1, 1), (2, 1), (2, 1), (2, 1), (3, 1), (3, 1), (4, 1)]
+H_SHELLS = [(0, 3), (0, 1), (0, 1), (1, 1), (1, 1), (2, 1), (3, 1)]
+
+
+@dataclass
+class Molecule:
+    """Shell batches of the config-5 molecule, one homogeneous batch per (l, K) type, and for every ordered pair of
+    types (la >= lb) the list of shell pairs (all pairs; i <= j inside one type)."""
+    positions: np.ndarray                 # [natom, 3]
+    types: list                           # [(l, K)] sorted
+    shells: dict                          # (l, K) -> Shells
+    atom_of: dict                         # (l, K) -> int array: atom index of each shell
+
+    def pair_types(self, lmax=4):
+        ts = [t for t in self.types if t[0] <= lmax]
+        return [(ta, tb) for i, ta in enumerate(ts) for tb in ts[: i + 1]]      # la >= lb (types sorted by l, K)
+
+    def pair_list(self, ta, tb):
+        na, nb = self.shells[ta].n, self.shells[tb].n
+        if ta == tb:
+            i, j = np.triu_indices(na)
+        else:
+            i, j = np.meshgrid(np.arange(na), np.arange(nb), indexing="ij")
+            i, j = i.ravel(), j.ravel()
+        return np.ascontiguousarray(np.stack([i, j], 1).astype(np.int32))
+
+    def nshells(self):
+        return sum(s.n for s in self.shells.values())
+
+    def nao(self, pure=True):
+        return sum(s.n * (nsolid(s.l) if pure else ncart(s.l)) for s in self.shells.values())
+
+
+def config5_molecule(n_heavy=48, n_h=96, edge=22.0, min_sep=1.8, seed=0):
+    """48 heavy + 96 H atoms at seeded random positions in a cube of `edge` bohr, rejection-sampled to a minimum
+    separation (reading S10); shells per atom as BASELINE.json lists them; exponents log-uniform in [0.1,5000] for
+    contracted shells and [0.1,10] for single primitives; coefficients per reading S11."""
+    rng = np.random.default_rng(seed)
+    pos = []
+    while len(pos) < n_heavy + n_h:
+        p = rng.uniform(0.0, edge, 3)
+        if all(np.linalg.norm(p - q) >= min_sep for q in pos):
+            pos.append(p)
+    pos = np.array(pos)
+    per_type = {}
+    for ia in range(n_heavy + n_h):
+        for (l, K) in (HEAVY_SHELLS if ia < n_heavy else H_SHELLS):
+            per_type.setdefault((l, K), []).append(ia)
+    types = sorted(per_type)
+    shells, atom_of = {}, {}
+    for t in types:
+        l, K = t
+        atoms = np.array(per_type[t])
+        zr = (0.1, 5000.0) if K > 1 else (0.1, 10.0)
+        s = make_shells(rng, len(atoms), l, K, zr, (0.0, 1.0))
+        s.center[:] = pos[atoms]
+        shells[t], atom_of[t] = s, atoms
+    return Molecule(pos, types, shells, atom_of)
+
+
+def config5_class(mol, tab, tcd, bra_pairs, ket_pairs, quartet_idx, name=None):
+    """One (la lb|lc ld) class of the molecule as a Workload: pair lists index into the type batches."""
+    (ta, tb), (tc, td) = tab, tcd
+    return Workload(name or f"cfg5_{ta}{tb}_{tc}{td}", mol.shells[ta], mol.shells[tb], mol.shells[tc], mol.shells[td],
+                    bra_pairs, ket_pairs, quartet_idx)
+
+
+def schwarz_count(qb, qk, thr, same):
+    """Number of (bra pair, ket pair) combinations with Q_bra Q_ket >= thr; `same`: the two lists are the same
+    pair type, count unordered combinations ij <= kl only."""
+    sk = np.sort(qk)
+    lo = np.searchsorted(sk, thr / np.maximum(qb, 1e-300), side="left")
+    n = int((len(sk) - lo).sum())
+    if same:
+        n = (n + int((qb * qb >= thr).sum())) // 2
+    return n
+
+
+def schwarz_sample(rng, qb, qk, thr, nsample, same):
+    """A seeded sample of quartet index pairs that pass the Schwarz bound (rejection sampling)."""
+    out = []
+    need = nsample
+    for _ in range(64):
+        if need <= 0:
+            break
+        i = rng.integers(0, len(qb), 2 * need + 16)
+        j = rng.integers(0, len(qk), 2 * need + 16)
+        ok = qb[i] * qk[j] >= thr
+        if same:
+            ok &= i <= j
+        sel = np.nonzero(ok)[0][:need]
+        out.append(np.stack([i[sel], j[sel]], 1))
+        need -= len(sel)
+    if not out:
+        return np.zeros((0, 2), np.int32)
+    return np.ascontiguousarray(np.concatenate(out).astype(np.int32))
