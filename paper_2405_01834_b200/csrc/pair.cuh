@@ -72,6 +72,13 @@ __global__ void __launch_bounds__(128) pair_setup_kernel(PairSetupArgs g) {
     double *E = sm;                     // [3][esz]
     double *T1 = sm + 3 * esz;          // [pchunk][nca][nb_out]
     __shared__ double hdr[5];           // p, P, coefficient
+    // Lane-varying reads of __constant__ tables serialise (one transaction per distinct address), which made this
+    // kernel 30x slower than its instruction count; the tables it needs are staged in shared memory instead.
+    __shared__ uint32_t s_herm[455];                  // N~(12): Hermite triples up to order la+lb <= 12
+    __shared__ double s_Ca[13 * 28], s_Cb[13 * 28];   // Cartesian -> solid matrices of the two shells
+    for (int i = threadIdx.x; i < nh; i += blockDim.x) s_herm[i] = c_herm[i];
+    for (int i = threadIdx.x; i < nsolid(la) * ncart(la); i += blockDim.x) s_Ca[i] = c_solid[solid_off(la) + i];
+    for (int i = threadIdx.x; i < nsolid(lb) * ncart(lb); i += blockDim.x) s_Cb[i] = c_solid[solid_off(lb) + i];
 
     const long long rid = blockIdx.x;   // pair * Ka*Kb + prim
     const long long ipair = rid / (Ka * Kb);
@@ -97,7 +104,7 @@ __global__ void __launch_bounds__(128) pair_setup_kernel(PairSetupArgs g) {
     if (threadIdx.x < 4) rec[threadIdx.x] = hdr[threadIdx.x];
     const double coef = hdr[4];
     const int nca = ncart(la), ncb = ncart(lb);
-    const uint32_t *ca = c_herm + nherm(la - 1), *cb = c_herm + nherm(lb - 1);   // component exponents
+    const uint32_t *ca = s_herm + nherm(la - 1), *cb = s_herm + nherm(lb - 1);   // component exponents
     const double *Ex = E, *Ey = E + esz, *Ez = E + 2 * esz;
     double *H = rec + 4;
 
@@ -106,7 +113,7 @@ __global__ void __launch_bounds__(128) pair_setup_kernel(PairSetupArgs g) {
         for (int e = threadIdx.x; e < nh * nab; e += blockDim.x) {
             int ih = e / nab, ab = e % nab, a = ab / ncb, b = ab % ncb;
             int t, u, v, ax, ay, az, bx, by, bz;
-            unpack_tuv(c_herm[ih], t, u, v);
+            unpack_tuv(s_herm[ih], t, u, v);
             unpack_tuv(ca[a], ax, ay, az);
             unpack_tuv(cb[b], bx, by, bz);
             double val = coef * Ex[(ax * (lb + 1) + bx) * nt + t] * Ey[(ay * (lb + 1) + by) * nt + u] *
@@ -122,7 +129,7 @@ __global__ void __launch_bounds__(128) pair_setup_kernel(PairSetupArgs g) {
         // zeros exactly (instead of leaving Eq. 17's cancellation to rounding) keeps the result accurate
         // relative to the small solid block (finding F1).
         const int nsa = nsolid(la), nlow = nherm(la - 1);
-        const double *Ca = c_solid + solid_off(la);
+        const double *Ca = s_Ca;
         double f = coef;
         for (int i = 0; i < la; ++i) f *= 0.5 / hdr[0];
         if (g.ket_sign && (la & 1)) f = -f;
@@ -132,39 +139,61 @@ __global__ void __launch_bounds__(128) pair_setup_kernel(PairSetupArgs g) {
         }
         return;
     }
-    // Solid harmonics, Eq. 17, one index at a time, pchunk Hermite rows per pass:
-    //   stage A  T1[p~][a][mb] = sum_b C^{lb}[mb][b] E^{ab}_{p~}
-    //   stage B  H[p~][ma][mb] = coef * sum_a C^{la}[ma][a] T1[p~][a][mb]
+    // Solid harmonics, Eq. 17, one index at a time, pchunk Hermite rows per pass, register-blocked:
+    //   stage A  thread (p~, a): the Cartesian row E^{ab}_{p~}, b = 0..ncb-1, in registers (Eq. 7, zeros by Eq. 14),
+    //            then T1[p~][a][mb] = sum_b C^{lb}[mb][b] E^{ab}_{p~}
+    //   stage B  thread (p~, mb): the column T1[p~][.][mb] in registers,
+    //            then H[p~][ma][mb] = coef * sum_a C^{la}[ma][a] T1[p~][a][mb]
+    constexpr int NCMAX = (MD_LMAX + 1) * (MD_LMAX + 2) / 2;
     const int nsa = nsolid(la), nsb = nsolid(lb);
-    const double *Ca = c_solid + solid_off(la), *Cb = c_solid + solid_off(lb);
+    const double *Ca = s_Ca, *Cb = s_Cb;
     for (int h0 = 0; h0 < nh; h0 += g.pchunk) {
         const int hc = min(g.pchunk, nh - h0);
-        for (int e = threadIdx.x; e < hc * nca * nsb; e += blockDim.x) {
-            int ih = e / (nca * nsb), r = e % (nca * nsb), a = r / nsb, mb = r % nsb;
+        for (int e = threadIdx.x; e < hc * nca; e += blockDim.x) {
+            const int ih = e / nca, a = e - ih * nca;
             int t, u, v, ax, ay, az;
-            unpack_tuv(c_herm[h0 + ih], t, u, v);
+            unpack_tuv(s_herm[h0 + ih], t, u, v);
             unpack_tuv(ca[a], ax, ay, az);
-            double s = 0.0;
-            for (int b = 0; b < ncb; ++b) {
-                double c = Cb[mb * ncb + b];
-                if (c == 0.0) continue;
-                int bx, by, bz;
-                unpack_tuv(cb[b], bx, by, bz);
-                if (t > ax + bx || u > ay + by || v > az + bz) continue;
-                s += c * Ex[(ax * (lb + 1) + bx) * nt + t] * Ey[(ay * (lb + 1) + by) * nt + u] *
-                     Ez[(az * (lb + 1) + bz) * nt + v];
+            const double *ex = Ex + ax * (lb + 1) * nt + t, *ey = Ey + ay * (lb + 1) * nt + u, *ez = Ez + az * (lb + 1) * nt + v;
+            double row[NCMAX];
+#pragma unroll
+            for (int b = 0; b < NCMAX; ++b) {
+                double x = 0.0;
+                if (b < ncb) {
+                    int bx, by, bz;
+                    unpack_tuv(cb[b], bx, by, bz);
+                    if (t <= ax + bx && u <= ay + by && v <= az + bz) x = ex[bx * nt] * ey[by * nt] * ez[bz * nt];
+                }
+                row[b] = x;
             }
-            T1[e] = s;
+            double *dst = T1 + (size_t)e * nsb;
+            for (int mb = 0; mb < nsb; ++mb) {
+                const double *c = Cb + mb * ncb;
+                double s0 = 0.0;
+#pragma unroll
+                for (int b = 0; b < NCMAX; ++b)
+                    if (b < ncb) s0 = fma(c[b], row[b], s0);
+                dst[mb] = s0;
+            }
         }
         __syncthreads();
-        for (int e = threadIdx.x; e < hc * nsa * nsb; e += blockDim.x) {
-            int ih = e / (nsa * nsb), r = e % (nsa * nsb), ma = r / nsb, mb = r % nsb;
-            const double *t1 = T1 + ih * nca * nsb + mb;
-            double s = 0.0;
-            for (int a = 0; a < nca; ++a) s += Ca[ma * nca + a] * t1[a * nsb];
-            s *= coef;
-            if (g.ket_sign && (c_herm[h0 + ih] >> 24 & 1)) s = -s;
-            H[(long long)(h0 + ih) * nsa * nsb + r] = s;
+        for (int e = threadIdx.x; e < hc * nsb; e += blockDim.x) {
+            const int ih = e / nsb, mb = e - ih * nsb;
+            const double *t1 = T1 + (size_t)ih * nca * nsb + mb;
+            double col[NCMAX];
+#pragma unroll
+            for (int a = 0; a < NCMAX; ++a) col[a] = a < nca ? t1[a * nsb] : 0.0;
+            const bool neg = g.ket_sign && (s_herm[h0 + ih] >> 24 & 1);
+            double *dst = H + (long long)(h0 + ih) * nsa * nsb + mb;
+            for (int ma = 0; ma < nsa; ++ma) {
+                const double *c = Ca + ma * nca;
+                double s0 = 0.0;
+#pragma unroll
+                for (int a = 0; a < NCMAX; ++a)
+                    if (a < nca) s0 = fma(c[a], col[a], s0);
+                s0 *= coef;
+                dst[(long long)ma * nsb] = neg ? -s0 : s0;
+            }
         }
         __syncthreads();
     }
