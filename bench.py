@@ -348,14 +348,14 @@ def run_config5(args):
             count = W.schwarz_count(Q[pb], Q[pk], thr, same)
             if count == 0:
                 continue
-            # The timed call sees a random subset of at most 512 pairs per side and a sample of the surviving quartets
+            # The timed call sees a random subset of at most 2048 pairs per side and a sample of the surviving quartets
             # among them: pair setup is then amortised over about as many quartets per pair as in the full sweep.
-            sb = np.sort(rng.choice(len(pairs[pb]), min(512, len(pairs[pb])), replace=False))
-            sk = sb if same else np.sort(rng.choice(len(pairs[pk]), min(512, len(pairs[pk])), replace=False))
+            sb = np.sort(rng.choice(len(pairs[pb]), min(2048, len(pairs[pb])), replace=False))
+            sk = sb if same else np.sort(rng.choice(len(pairs[pk]), min(2048, len(pairs[pk])), replace=False))
             qb_s, qk_s = Q[pb][sb], Q[pk][sk]
             avail = W.schwarz_count(qb_s, qk_s, thr, same)
             if avail == 0:                                   # the subset happens to hold no surviving quartet
-                sb = np.argsort(-Q[pb])[:512]; sk = sb if same else np.argsort(-Q[pk])[:512]
+                sb = np.argsort(-Q[pb])[:2048]; sk = sb if same else np.argsort(-Q[pk])[:2048]
                 sb, sk = np.sort(sb), np.sort(sk)
                 qb_s, qk_s = Q[pb][sb], Q[pk][sk]
                 avail = W.schwarz_count(qb_s, qk_s, thr, same)

@@ -92,7 +92,7 @@ cudaError_t mma_launch(const MmaCall &c, int nsm, cudaStream_t st, int *info) {
         k.ctas = k.smem <= (size_t)(g_max_smem + 1024) / 2 - 1024 ? 2 : 1;
         // prefer two CTAs per SM unless one CTA saves more than a third of the warp-steps
         auto score = [](const Cand &x) { return (double)x.cost * (x.ctas == 2 ? 1.0 : 1.35); };
-        if (!have || score(k) < score(best) - 1e-9) { best = k; have = true; }
+        if (!have || score(k) <= score(best) + 1e-9) { best = k; have = true; }   // ties: the larger row block reuses each B fragment more
     }
     if (!have) return cudaErrorInvalidConfiguration;
 
