@@ -48,7 +48,7 @@ cudaError_t mma_launch(const MmaCall &c, int nsm, cudaStream_t st, int *info) {
 
     // Candidate row-block shapes: one per MW.  cost = warp-steps of GEMM1 per pass (8 m-tiles run abreast),
     // smem decides how many CTAs share an SM.
-    struct Cand { int MW, nkb, np, cached, rslots; long long cost; size_t smem; int ctas; };
+    struct Cand { int MW, nkb, np, cached, rslots, nblocks; long long cost; size_t smem; int ctas; };
     Cand best{};
     bool have = false;
     for (int MW = 1; MW <= MWMAX; ++MW) {
@@ -60,6 +60,7 @@ cudaError_t mma_launch(const MmaCall &c, int nsm, cudaStream_t st, int *info) {
             k.nkb = 1;
             k.np = std::min(cap, ((nhb + nblk - 1) / nblk + 7) / 8 * 8);
             const int nb = (nhb + k.np - 1) / k.np;
+            k.nblocks = nb * c.Kbra;
             k.cost = 0;
             for (int b = 0; b < nb; ++b) {
                 const int rows = std::min(k.np, nhb - b * k.np);
@@ -71,6 +72,7 @@ cudaError_t mma_launch(const MmaCall &c, int nsm, cudaStream_t st, int *info) {
             const int nblk = (c.Kbra + fit - 1) / fit;
             k.nkb = (c.Kbra + nblk - 1) / nblk;
             k.np = nhb;
+            k.nblocks = nblk;
             k.cost = 0;
             for (int b = 0; b < nblk; ++b) {
                 const int rows = std::min(k.nkb, c.Kbra - b * k.nkb) * nhb;
@@ -92,7 +94,9 @@ cudaError_t mma_launch(const MmaCall &c, int nsm, cudaStream_t st, int *info) {
         k.ctas = k.smem <= (size_t)(g_max_smem + 1024) / 2 - 1024 ? 2 : 1;
         // prefer two CTAs per SM unless one CTA saves more than a third of the warp-steps
         auto score = [](const Cand &x) { return (double)x.cost * (x.ctas == 2 ? 1.0 : 1.35); };
-        if (!have || score(k) <= score(best) + 1e-9) { best = k; have = true; }   // ties: the larger row block reuses each B fragment more
+        // ties: fewer row blocks (each B fragment is reused by more row tiles), then the smaller tile
+        const double d = score(k) - score(best);
+        if (!have || d < -1e-9 || (d <= 1e-9 && k.nblocks < best.nblocks)) { best = k; have = true; }
     }
     if (!have) return cudaErrorInvalidConfiguration;
 
