@@ -2,6 +2,7 @@
 // variant selection and kernel launches.  No integral arithmetic runs on the host; the only
 // host-computed numbers are the constant index / solid-harmonic coefficient tables uploaded
 // once by md_init().
+#include <algorithm>
 #include <cmath>
 #include <cstdio>
 #include <cstring>
@@ -147,7 +148,15 @@ int launch_pair_setup(const PairView &pv, int pure, int ket_sign, long long stri
     size_t smem = 8 * ((size_t)3 * esz + (pure ? (size_t)a.pchunk * rowsz : 0));
     long long nblk = pv.npairs * Kab;
     if (nblk > 0x7fffffffLL) return MD_EINVAL;
-    pair_setup_kernel<<<(unsigned)nblk, 128, smem, st>>>(a);
+    switch (std::max(la, lb)) {
+        case 0: pair_setup_kernel<0><<<(unsigned)nblk, 128, smem, st>>>(a); break;
+        case 1: pair_setup_kernel<1><<<(unsigned)nblk, 128, smem, st>>>(a); break;
+        case 2: pair_setup_kernel<2><<<(unsigned)nblk, 128, smem, st>>>(a); break;
+        case 3: pair_setup_kernel<3><<<(unsigned)nblk, 128, smem, st>>>(a); break;
+        case 4: pair_setup_kernel<4><<<(unsigned)nblk, 128, smem, st>>>(a); break;
+        case 5: pair_setup_kernel<5><<<(unsigned)nblk, 128, smem, st>>>(a); break;
+        default: pair_setup_kernel<6><<<(unsigned)nblk, 128, smem, st>>>(a); break;
+    }
     S.last_launches++;
     CK(cudaGetLastError());
     return MD_OK;
@@ -280,7 +289,13 @@ int md_init(void) {
     CK(cudaDeviceGetAttribute(&S.nsm, cudaDevAttrMultiProcessorCount, dev));
     CK(cudaDeviceGetAttribute(&S.max_smem, cudaDevAttrMaxSharedMemoryPerBlockOptin, dev));
     CK(cudaFuncSetAttribute(eri_generic_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, S.max_smem - 1024));
-    CK(cudaFuncSetAttribute(pair_setup_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, 96 * 1024));
+    CK(cudaFuncSetAttribute(pair_setup_kernel<0>, cudaFuncAttributeMaxDynamicSharedMemorySize, 96 * 1024));
+    CK(cudaFuncSetAttribute(pair_setup_kernel<1>, cudaFuncAttributeMaxDynamicSharedMemorySize, 96 * 1024));
+    CK(cudaFuncSetAttribute(pair_setup_kernel<2>, cudaFuncAttributeMaxDynamicSharedMemorySize, 96 * 1024));
+    CK(cudaFuncSetAttribute(pair_setup_kernel<3>, cudaFuncAttributeMaxDynamicSharedMemorySize, 96 * 1024));
+    CK(cudaFuncSetAttribute(pair_setup_kernel<4>, cudaFuncAttributeMaxDynamicSharedMemorySize, 96 * 1024));
+    CK(cudaFuncSetAttribute(pair_setup_kernel<5>, cudaFuncAttributeMaxDynamicSharedMemorySize, 96 * 1024));
+    CK(cudaFuncSetAttribute(pair_setup_kernel<6>, cudaFuncAttributeMaxDynamicSharedMemorySize, 96 * 1024));
     CK(fused_init(S.max_smem));
     CK(fused2_init(S.max_smem));
     CK(mma_init(S.max_smem));

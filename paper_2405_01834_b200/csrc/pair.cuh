@@ -62,6 +62,8 @@ struct PairSetupArgs {
 };
 
 // One CTA per (pair, primitive pair).  Shared memory: 3 axis tables + the stage-A buffer.
+// LM = max(la, lb) sizes the register rows of the solid transform (one instantiation per LM).
+template <int LM>
 __global__ void __launch_bounds__(128) pair_setup_kernel(PairSetupArgs g) {
     extern __shared__ double sm[];
     const PairView &pv = g.pv;
@@ -144,7 +146,7 @@ __global__ void __launch_bounds__(128) pair_setup_kernel(PairSetupArgs g) {
     //            then T1[p~][a][mb] = sum_b C^{lb}[mb][b] E^{ab}_{p~}
     //   stage B  thread (p~, mb): the column T1[p~][.][mb] in registers,
     //            then H[p~][ma][mb] = coef * sum_a C^{la}[ma][a] T1[p~][a][mb]
-    constexpr int NCMAX = (MD_LMAX + 1) * (MD_LMAX + 2) / 2;
+    constexpr int NCMAX = (LM + 1) * (LM + 2) / 2;
     const int nsa = nsolid(la), nsb = nsolid(lb);
     const double *Ca = s_Ca, *Cb = s_Cb;
     for (int h0 = 0; h0 < nh; h0 += g.pchunk) {
