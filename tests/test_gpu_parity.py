@@ -152,6 +152,34 @@ def test_fused2_mixed_contraction_and_clustered():
         check(W.clustered((2, 2, 2, 2), 29, K=(2, 2, 2, 2), coincide=coincide), True, FUSED2)
 
 
+def test_fused2_is_deterministic():
+    """Named-barrier hand-over, aliased drain region, L2 scratch: a race would show up as run-to-run differences."""
+    for w, pure in [(W.config2(K=3, n=2500), True), (W.class_sweep((2, 1, 2, 0), 3001, K=(2, 2, 3, 1)), False)]:
+        ref, used = gpu_run(w, pure, FUSED2)
+        assert used == FUSED2
+        for _ in range(3):
+            again, _ = gpu_run(w, pure, FUSED2)
+            assert np.array_equal(ref, again)
+
+
+@pytest.mark.parametrize("ls", [(1, 1, 1, 1), (2, 0, 1, 1), (1, 1, 2, 0), (2, 1, 2, 2), (2, 2, 2, 0), (0, 2, 1, 2), (1, 2, 1, 1)],
+                         ids=lambda ls: "".join(map(str, ls)))
+def test_fused2_every_registered_shape(ls):
+    """The other instantiated classes (la+lb >= 2, lc+ld >= 2), canonical and swapped shell order, contracted."""
+    w = W.independent_quartets("f2cls", ls, (2, 1, 3, 2), 157, (0.05, 50.0), (-3.0, 3.0), W.class_seed("f2cls", ls))
+    for pure in (True, False):
+        _, used = check(w, pure, FUSED2)
+        assert used == FUSED2
+    check(W.clustered(ls, 23, K=(1, 2, 2, 1)), True, FUSED2)
+
+
+def test_fused2_three_center_with_d_fitting_shell():
+    w = W.class_sweep((2, 1, 2), 211, K=(3, 2, 1), three_center=True)
+    for pure in (True, False):
+        _, used = check(w, pure, FUSED2)
+        assert used == FUSED2
+
+
 def test_fused2_product_mode_and_paper_layout():
     w = _product((2, 2, 2, 2), 11, 6, K=3)
     for pure in (True, False):
