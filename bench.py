@@ -294,6 +294,22 @@ def sweep_cases(name):
                     la, lb, lX, K=K, n=200_000), True, ("auto",)))
         for ls in [(3, 3, 3, 3), (4, 4, 4, 4), (5, 5, 5, 5), (6, 6, 6, 6), (3, 4, 5, 6)]:
             cases.append((f"cfg4 ({ls[0]}{ls[1]}|{ls[2]}{ls[3]}) K=1 solid", lambda ls=ls: W.config4(ls, n=20_000), True, ("auto",)))
+    elif name == "all":              # sweep 6 of SURVEY.md 8(d): every canonical class, K = 1, config-4 distribution
+        pairs = [(a, b) for a in range(7) for b in range(a + 1)]
+        for ib, b in enumerate(pairs):
+            for k in pairs[: ib + 1]:
+                ls = b + k
+                nout = 1
+                for l in ls:
+                    nout *= 2 * l + 1
+                n = int(min(200_000, (1 << 30) // (8 * nout)))
+                cases.append((f"({b[0]}{b[1]}|{k[0]}{k[1]})", lambda ls=ls, n=n: W.class_sweep(ls, n), True, ("auto",)))
+        for b in pairs:
+            for lX in range(7):
+                nout = (2 * b[0] + 1) * (2 * b[1] + 1) * (2 * lX + 1)
+                n = int(min(200_000, (1 << 30) // (8 * nout)))
+                cases.append((f"({b[0]}{b[1]}|{lX})", lambda b=b, lX=lX, n=n: W.class_sweep(b + (lX,), n, K=(1, 1, 1),
+                                                                                             three_center=True), True, ("auto",)))
     else:
         raise SystemExit(f"unknown sweep {name!r}")
     return cases
@@ -422,7 +438,7 @@ def run_sweep(args):
                                        np.stack([np.arange(1000, dtype=np.int32)] * 2, 1))
                     dp = engine.DeviceWorkload(probe); op = dp.alloc_out(pure)
                     ms_p = time_steps(lambda: dp.run(pure, op), 2, 2, flush, lambda: None) / 2
-                    cap = int(max(2000, min(w.nquartets, 1000 * 400.0 / max(ms_p, 1e-3))))   # about 0.4 s per step
+                    cap = int(max(2000, min(w.nquartets, 1000 * (100.0 if args.sweep == 'all' else 400.0) / max(ms_p, 1e-3))))   # about 0.4 s per step (0.1 s in the 602-class sweep)
                     if cap < w.nquartets:
                         sel = np.arange(cap)
                         ia, ib, ic, id_ = w.shell_indices(sel)
@@ -453,7 +469,7 @@ def main():
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--variants", action="store_true", help="also time K=1 and Cartesian output")
     ap.add_argument("--cpu-sample", type=int, default=8000)
-    ap.add_argument("--sweep", default=None, help="per-class table instead of the headline: l2 | configs | config5")
+    ap.add_argument("--sweep", default=None, help="per-class table instead of the headline: l2 | configs | config5 | all")
     args = ap.parse_args()
     args.warmup = max(args.warmup, 3) if args.impl == "ours" else args.warmup
     if args.sweep:
