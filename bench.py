@@ -156,7 +156,7 @@ def measure_variant(dw, w, K, pure, steps, warmup, flush, barrier):
     flops = W.flops_model(2, 2, 2, 2, K * K, K * K, pure)
     return {"K": K, "pure": pure, "ms_per_step": ms / steps, "quartets_per_s": w.nquartets * steps / (ms * 1e-3),
             "model_flop_per_quartet": flops, "model_tflops": flops * w.nquartets * steps / (ms * 1e-3) / 1e12,
-            "variant": {1: "generic", 2: "fused", 3: "mma", 4: "fused2"}.get(engine.md_last_variant(), "?"),
+            "variant": {1: "generic", 2: "fused", 3: "mma", 4: "fused2", 5: "warp"}.get(engine.md_last_variant(), "?"),
             "launches_per_step": engine.md_last_launch_count(), "out_bytes": out.numel() * 8}
 
 
@@ -310,6 +310,26 @@ def sweep_cases(name):
                 n = int(min(200_000, (1 << 30) // (8 * nout)))
                 cases.append((f"({b[0]}{b[1]}|{lX})", lambda b=b, lX=lX, n=n: W.class_sweep(b + (lX,), n, K=(1, 1, 1),
                                                                                              three_center=True), True, ("auto",)))
+    elif name == "paper":            # sweep 7: the paper's Tables IV and V shapes, bra list x ket list products
+        def size(ls, Kb, Kk, three):
+            nout = 1
+            for l in ls:
+                nout *= 2 * l + 1
+            fl = W.flops_model(ls[0], ls[1], ls[2], 0 if three else ls[3], Kb, Kk, True)
+            n = min(1_000_000, (1 << 30) // (8 * nout), int(6e11 / fl))
+            return max(8, int(n ** 0.5))
+        four = [(l, l, 0, 0) for l in range(1, 7)] + [(l, 0, l, 0) for l in range(1, 7)] + [(l, l, l, l) for l in range(7)]
+        for ls in four:
+            for Kb, Kk in ((1, 1), (1, 5), (5, 5)):      # the paper sorts the higher contraction onto the ket
+                m = size(ls, Kb, Kk, False)
+                cases.append((f"[{ls[0]}{ls[1]}|{ls[2]}{ls[3]}] {{{Kb};{Kk}}}", lambda ls=ls, Kb=Kb, Kk=Kk, m=m: W.paper_microbench(
+                    ls, Kb, Kk, m, m), True, ("auto",)))
+        three = [(0, 0, l) for l in range(1, 7)] + [(l, l, 0) for l in range(1, 7)] + [(l, l, l) for l in range(7)]
+        for ls in three:                                 # the paper's [a|cd] {Ka;Kcd} is (cd|a) here: pair first
+            for Ka, Kcd in ((1, 1), (1, 5), (5, 5)):
+                m = size(ls, Kcd, Ka, True)
+                cases.append((f"[{ls[2]}|{ls[0]}{ls[1]}] {{{Ka};{Kcd}}}", lambda ls=ls, Ka=Ka, Kcd=Kcd, m=m: W.paper_microbench(
+                    ls, Kcd, Ka, m, m, three_center=True), True, ("auto",)))
     else:
         raise SystemExit(f"unknown sweep {name!r}")
     return cases
@@ -352,7 +372,7 @@ def run_config5(args):
     Q = {pt: schwarz_factors(engine, W, mol, pt[0], pt[1], pairs[pt]) for pt in ptypes}
     torch.cuda.synchronize()
     t_schwarz = time.perf_counter() - t0
-    vname = {1: "generic", 2: "fused", 3: "mma", 4: "fused2"}
+    vname = {1: "generic", 2: "fused", 3: "mma", 4: "fused2", 5: "warp"}
     rows = ["class,Kbra,Kket,pairs_bra,pairs_ket,quartets_passing,sampled,variant,ms,quartets_per_s,model_tflops,"
             "extrapolated_s"]
     rng = np.random.default_rng(5)
@@ -414,8 +434,8 @@ def run_sweep(args):
     engine.md_init()
     flush = torch.empty(256 << 20, dtype=torch.uint8, device="cuda")
     vid = {"auto": engine.VARIANT_AUTO, "generic": engine.VARIANT_GENERIC, "fused": engine.VARIANT_FUSED,
-           "mma": engine.VARIANT_MMA, "fused2": engine.VARIANT_FUSED2}
-    vname = {1: "generic", 2: "fused", 3: "mma", 4: "fused2"}
+           "mma": engine.VARIANT_MMA, "fused2": engine.VARIANT_FUSED2, "warp": engine.VARIANT_WARP}
+    vname = {1: "generic", 2: "fused", 3: "mma", 4: "fused2", 5: "warp"}
     try:
         hbm = json.load(open(os.path.join(ROOT, "MEASURED_PEAKS.json"))).get("hbm_gbs", 6550.0)
     except (OSError, ValueError):
@@ -430,7 +450,7 @@ def run_sweep(args):
             engine.md_set_variant(vid[v])
             try:
                 ww = w
-                if w.nquartets > 2000:                     # bound the time per case: probe on 1000 quartets first
+                if w.nquartets > 2000 and w.quartet_idx is not None:   # bound the time per case: probe on 1000 quartets first
                     sel = np.arange(1000)
                     probe = W.Workload("probe", w.a.take(w.shell_indices(sel)[0]), w.b.take(w.shell_indices(sel)[1]),
                                        w.c.take(w.shell_indices(sel)[2]),
@@ -469,7 +489,7 @@ def main():
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--variants", action="store_true", help="also time K=1 and Cartesian output")
     ap.add_argument("--cpu-sample", type=int, default=8000)
-    ap.add_argument("--sweep", default=None, help="per-class table instead of the headline: l2 | configs | config5 | all")
+    ap.add_argument("--sweep", default=None, help="per-class table instead of the headline: l2 | configs | config5 | all | paper")
     args = ap.parse_args()
     args.warmup = max(args.warmup, 3) if args.impl == "ours" else args.warmup
     if args.sweep:

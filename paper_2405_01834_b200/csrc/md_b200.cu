@@ -15,6 +15,7 @@
 #include "generic.cuh"
 #include "mma_api.cuh"
 #include "pair.cuh"
+#include "warp.cuh"
 #include "peak.cuh"
 
 using namespace mdb;
@@ -200,6 +201,24 @@ int run_generic(const PairView &b, const PairView &k, long long nq, const int32_
     ct = std::min<long long>(ct, std::max(16, 4096 / s.nhb));
     g.ct = (int)std::min<long long>(ct, s.ncd);
     size_t smem = fixed + 8 * (size_t)s.nhb * g.ct;
+    // Small classes: one warp per quartet (warp.cuh) instead of one CTA per quartet.
+    const int kq0 = (k.single && pure) ? nherm(k.a.l - 1) : 0;
+    if (use_mma && S.variant != MD_VARIANT_MMA && g.Lb + g.Lk <= MD_WARP_LMAX && s.nhb * s.ncd <= MD_WARP_HALF) {
+        WarpArgs w;
+        w.rec_bra = rec_b; w.rec_ket = rec_k; w.stride_bra = s.stride_b; w.stride_ket = s.stride_k;
+        w.Kbra = g.Kbra; w.Kket = g.Kket; w.Lb = g.Lb; w.Lk = g.Lk; w.nab = s.nab; w.ncd = s.ncd; w.kq0 = kq0;
+        w.qidx = qidx; w.nq = nq; w.nket = k.npairs; w.out = out;
+        w.s_q = g.s_q; w.s_bi = g.s_bi; w.s_ki = g.s_ki; w.s_ab = g.s_ab; w.s_cd = g.s_cd;
+        w.boys_tab = S.boys_tab; w.rlut = fused_rlut();
+        const size_t wsm = 8 * (size_t)(MD_WARP_THREADS / 32) * warp_smem_doubles(g.Lb + g.Lk, s.nhb, s.ncd);
+        const long long nblk = (nq + MD_WARP_THREADS / 32 - 1) / (MD_WARP_THREADS / 32);
+        const unsigned wgrid = (unsigned)std::min<long long>(nblk, (long long)S.nsm * 8);
+        eri_warp_kernel<<<wgrid, MD_WARP_THREADS, wsm, st>>>(w);
+        S.last_launches++;
+        CK(cudaGetLastError());
+        S.last_variant = MD_VARIANT_WARP;
+        return MD_OK;
+    }
     if (use_mma) {
         MmaCall c;
         c.rec_bra = rec_b; c.rec_ket = rec_k; c.stride_bra = s.stride_b; c.stride_ket = s.stride_k;
@@ -296,6 +315,7 @@ int md_init(void) {
     CK(cudaFuncSetAttribute(pair_setup_kernel<4>, cudaFuncAttributeMaxDynamicSharedMemorySize, 96 * 1024));
     CK(cudaFuncSetAttribute(pair_setup_kernel<5>, cudaFuncAttributeMaxDynamicSharedMemorySize, 96 * 1024));
     CK(cudaFuncSetAttribute(pair_setup_kernel<6>, cudaFuncAttributeMaxDynamicSharedMemorySize, 96 * 1024));
+    CK(cudaFuncSetAttribute(eri_warp_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, 96 * 1024));
     CK(fused_init(S.max_smem));
     CK(fused2_init(S.max_smem));
     CK(mma_init(S.max_smem));
@@ -350,7 +370,7 @@ int md_set_workspace(void *p, size_t bytes) {
     return MD_OK;
 }
 int md_set_variant(int v) {
-    if (v < MD_VARIANT_AUTO || v > MD_VARIANT_FUSED2) return MD_EINVAL;
+    if (v < MD_VARIANT_AUTO || v > MD_VARIANT_WARP) return MD_EINVAL;
     S.variant = v;
     return MD_OK;
 }

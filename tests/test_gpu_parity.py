@@ -193,6 +193,43 @@ def test_fused2_product_mode_and_paper_layout():
         assert_parity(v, ref, "fused2 paper layout")
 
 
+# ---- the one-warp-per-quartet kernel for small classes -------------------------------------------------------
+
+WARP = engine.VARIANT_WARP
+
+
+@pytest.mark.parametrize("ls", [(3, 0, 0, 0), (0, 0, 0, 3), (3, 3, 0, 0), (0, 0, 3, 3), (3, 0, 3, 0), (4, 0, 4, 0), (4, 4, 0, 0),
+                                (3, 2, 1, 0), (0, 3, 2, 1), (5, 0, 1, 0), (6, 0, 0, 0), (4, 1, 1, 1)], ids=lambda ls: "".join(map(str, ls)))
+def test_warp_kernel_four_center(ls):
+    for pure in (True, False):
+        _, used = check(W.class_sweep(ls, 203), pure, WARP)
+        assert used == WARP
+        check(W.clustered(ls, 31, K=(2, 1, 1, 3)), pure, WARP)
+    _, used = check(W.class_sweep(ls, 97), True)          # MD_VARIANT_AUTO picks it for these classes
+    assert used == WARP
+
+
+@pytest.mark.parametrize("la,lb,lX", [(0, 0, 3), (0, 0, 6), (1, 0, 4), (3, 3, 0), (4, 4, 0), (3, 1, 2), (2, 2, 4), (0, 3, 5)])
+def test_warp_kernel_three_center(la, lb, lX):
+    for pure in (True, False):
+        _, used = check(W.class_sweep((la, lb, lX), 203, K=(2, 2, 1), three_center=True), pure, WARP)
+        assert used == WARP
+
+
+def test_warp_kernel_product_mode_and_paper_layout():
+    for ls, three in [((3, 0, 3, 0), False), ((0, 0, 4), True)]:
+        w = _product(ls, 13, 7, three_center=three, K=2)
+        ref = oracle_run(w, True)
+        gpu, used = gpu_run(w, True, WARP)
+        assert used == WARP
+        assert_parity(gpu.reshape(ref.shape), ref, "warp product")
+        gp, _ = gpu_run(w, True, WARP, layout=engine.LAYOUT_PAPER)
+        nab = engine.ncomp(ls[0], True) * engine.ncomp(ls[1], True)
+        ncd = engine.ncomp(ls[2], True) * (1 if three else engine.ncomp(ls[3], True))
+        v = gp.reshape(7, ncd, nab, 13).transpose(3, 0, 2, 1).reshape(13 * 7, nab * ncd)
+        assert_parity(v, ref, "warp paper layout")
+
+
 # ---- 3-center ----------------------------------------------------------------------------------------------
 
 @pytest.mark.parametrize("la,lb,lX", [(0, 0, 0), (1, 0, 0), (0, 1, 2), (1, 1, 1), (2, 2, 2), (2, 0, 6), (3, 3, 6), (3, 1, 4),
