@@ -315,7 +315,7 @@ int md_init(void) {
     CK(cudaFuncSetAttribute(pair_setup_kernel<4>, cudaFuncAttributeMaxDynamicSharedMemorySize, 96 * 1024));
     CK(cudaFuncSetAttribute(pair_setup_kernel<5>, cudaFuncAttributeMaxDynamicSharedMemorySize, 96 * 1024));
     CK(cudaFuncSetAttribute(pair_setup_kernel<6>, cudaFuncAttributeMaxDynamicSharedMemorySize, 96 * 1024));
-    CK(cudaFuncSetAttribute(eri_warp_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, 96 * 1024));
+    CK(cudaFuncSetAttribute(eri_warp_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, 112 * 1024));
     CK(fused_init(S.max_smem));
     CK(fused2_init(S.max_smem));
     CK(mma_init(S.max_smem));

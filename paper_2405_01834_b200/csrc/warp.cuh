@@ -6,7 +6,7 @@
 // Here each warp owns a quartet: the lanes evaluate F_m(T) for m = 0..L (one order per lane), build the
 // Hermite Coulomb tensor level by level in the warp's own shared memory (Eqs. 21-24, __syncwarp only),
 // and run the two Hermite->AO contractions (Eqs. 19, 25, 26) as DFMA loops over the dense H matrices of
-// pair_setup_kernel, one output element per lane at a time.  L = la+lb+lc+ld <= 8.
+// pair_setup_kernel, one output element per lane at a time.  L = la+lb+lc+ld <= 12.
 #pragma once
 #include "boys.cuh"
 #include "common.cuh"
@@ -15,7 +15,7 @@
 namespace mdb {
 
 #define MD_WARP_THREADS 256
-#define MD_WARP_LMAX 8
+#define MD_WARP_LMAX 12
 #define MD_WARP_HALF 640                 // largest [p~|cd] block (doubles) a warp keeps
 
 struct WarpArgs {
@@ -40,7 +40,7 @@ __host__ __device__ inline int warp_smem_doubles(int L, int nhb, int ncd) {
 
 __global__ void __launch_bounds__(MD_WARP_THREADS) eri_warp_kernel(WarpArgs g) {
     extern __shared__ double sm[];
-    __shared__ uint32_t s_w[165];                              // packed (t,u,v,n) of the first N~(8) Hermite triples
+    __shared__ uint32_t s_w[455];                              // packed (t,u,v,n) of the first N~(12) Hermite triples
     const int L = g.Lb + g.Lk, nhb = nherm(g.Lb), nhk = nherm(g.Lk);
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5, nwarp = MD_WARP_THREADS / 32;
     const uint2 *lut = (const uint2 *)g.rlut;
