@@ -255,6 +255,11 @@ int run(const PairView &b, const PairView &k, long long nq, const int32_t *qidx,
     if (e) return e;
     S.last_launches = 0;
     if (nq == 0) return MD_OK;
+    // Measured exception: a bra x ket PRODUCT with an s-type ket ((dd|ss), (dd|s)) amortises pair
+    // setup over the whole ket list, and the one-warp-per-quartet kernel is then 2-3.5x faster than the fused one.
+    const bool product_s_ket = S.variant == MD_VARIANT_AUTO && !qidx && k.a.l == 0 && (k.single || k.b.l == 0) &&
+                               b.a.l + (b.single ? 0 : b.b.l) >= 4 && nq >= 8 * (b.npairs + k.npairs);
+    if (product_s_ket) return run_generic(b, k, nq, qidx, pure, layout, out, st, true);
     if (S.variant == MD_VARIANT_AUTO || S.variant == MD_VARIANT_FUSED2) {
         // By measurement (profiles/r01_sweep_l2.md): the warp-specialised kernel wins on every instantiated class
         // once the primitive loop is long enough to fill its pipeline, and on (dd|dd) for any K.

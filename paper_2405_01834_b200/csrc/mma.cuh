@@ -21,8 +21,8 @@
 
 namespace mdb {
 
-#define MD_MMA_THREADS 256
-#define MD_MMA_WARPS 8
+// CTA size is a template parameter (4 or 8 warps): small classes run faster with four CTAs of 4 warps per SM,
+// the largest ones with two CTAs of 8 warps (measured; the host picks, mma_inst.cu).
 
 struct MmaArgs {
     const double *rec_bra, *rec_ket;     // pair_setup_kernel records
@@ -54,9 +54,9 @@ __device__ __forceinline__ int herm_index_packed(uint32_t w) {
     return ((n * (n + 1) * (n + 2) * 10923) >> 16) + ((a * (a + 1)) >> 1) + v;
 }
 
-template <int MW, int NW>
+template <int MW, int NW, int MD_MMA_WARPS>
 struct MmaCfg {
-    static constexpr int ROWS = 64 * MW;            // stacked rows per row-block
+    static constexpr int ROWS = 8 * MD_MMA_WARPS * MW;            // stacked rows per row-block
     static constexpr int NT = 8 * NW;               // cd columns per pass
     static constexpr int NTS = NT + 4;              // row stride of [p~|cd]: conflict-free B-fragment loads
 };
@@ -83,9 +83,10 @@ __host__ __device__ inline MmaSmem mma_smem_layout(int L, int rslots, int Kbra, 
     return s;
 }
 
-template <int MW, int NW>
-__global__ void __launch_bounds__(MD_MMA_THREADS, 2) eri_mma_kernel(MmaArgs g) {
-    using C = MmaCfg<MW, NW>;
+template <int MW, int NW, int MD_MMA_WARPS>
+__global__ void __launch_bounds__(32 * MD_MMA_WARPS, 16 / MD_MMA_WARPS) eri_mma_kernel(MmaArgs g) {
+    constexpr int MD_MMA_THREADS = 32 * MD_MMA_WARPS;
+    using C = MmaCfg<MW, NW, MD_MMA_WARPS>;
     extern __shared__ double sm[];
     const int L = g.Lb + g.Lk;
     const int nhb = nherm(g.Lb), nhk = nherm(g.Lk);

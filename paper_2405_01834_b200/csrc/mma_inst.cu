@@ -10,13 +10,16 @@ namespace {
 
 constexpr int MWMAX = 5, NWMAX = 4;
 typedef void (*MmaFn)(MmaArgs);
-MmaFn g_fn[MWMAX + 1][NWMAX + 1];
+MmaFn g_fn[2][MWMAX + 1][NWMAX + 1];      // [0]: 4-warp CTAs, [1]: 8-warp CTAs
 int g_max_smem = 227 * 1024;
 
 template <int MW, int NW>
 cudaError_t reg1(int max_smem) {
-    g_fn[MW][NW] = eri_mma_kernel<MW, NW>;
-    return cudaFuncSetAttribute(eri_mma_kernel<MW, NW>, cudaFuncAttributeMaxDynamicSharedMemorySize, max_smem - 1024);
+    g_fn[0][MW][NW] = eri_mma_kernel<MW, NW, 4>;
+    g_fn[1][MW][NW] = eri_mma_kernel<MW, NW, 8>;
+    cudaError_t e = cudaFuncSetAttribute(eri_mma_kernel<MW, NW, 4>, cudaFuncAttributeMaxDynamicSharedMemorySize, max_smem - 1024);
+    if (e != cudaSuccess) return e;
+    return cudaFuncSetAttribute(eri_mma_kernel<MW, NW, 8>, cudaFuncAttributeMaxDynamicSharedMemorySize, max_smem - 1024);
 }
 template <int MW>
 cudaError_t reg_row(int max_smem) {
@@ -48,11 +51,16 @@ cudaError_t mma_launch(const MmaCall &c, int nsm, cudaStream_t st, int *info) {
 
     // Candidate row-block shapes: one per MW.  cost = warp-steps of GEMM1 per pass (8 m-tiles run abreast),
     // smem decides how many CTAs share an SM.
-    struct Cand { int MW, nkb, np, cached, rslots, nblocks; long long cost; size_t smem; int ctas; };
+    struct Cand { int MW, nkb, np, cached, rslots, nblocks, warps; long long cost; size_t smem; int ctas; };
     Cand best{};
     bool have = false;
+    // CTA size by measurement: four CTAs of 4 warps per SM for the smaller classes ((ff|ff) 5.5 -> 4.6 ms per 20,000,
+    // (fd|dp) 3.7 -> 2.6 ms per 50,000), two CTAs of 8 warps for the large ones ((gg|gg), (ii|ii), (fg|hi) lose 10-40 %
+    // with 4 warps); then the row-block shape.
+    const bool small = nhb <= 128 && c.ncd <= 64;
+    for (int MD_MMA_WARPS = small ? 4 : 8; MD_MMA_WARPS <= 8 && !have; MD_MMA_WARPS += 4)
     for (int MW = 1; MW <= MWMAX; ++MW) {
-        const int cap = 64 * MW;
+        const int cap = 8 * MD_MMA_WARPS * MW;
         Cand k{};
         k.MW = MW;
         if (nhb > cap) {
@@ -64,7 +72,7 @@ cudaError_t mma_launch(const MmaCall &c, int nsm, cudaStream_t st, int *info) {
             k.cost = 0;
             for (int b = 0; b < nb; ++b) {
                 const int rows = std::min(k.np, nhb - b * k.np);
-                k.cost += ((rows + 7) / 8 + 7) / 8;
+                k.cost += ((rows + 7) / 8 + MD_MMA_WARPS - 1) / MD_MMA_WARPS;
             }
             k.cost *= c.Kbra;
         } else {
@@ -76,7 +84,7 @@ cudaError_t mma_launch(const MmaCall &c, int nsm, cudaStream_t st, int *info) {
             k.cost = 0;
             for (int b = 0; b < nblk; ++b) {
                 const int rows = std::min(k.nkb, c.Kbra - b * k.nkb) * nhb;
-                k.cost += ((rows + 7) / 8 + 7) / 8;
+                k.cost += ((rows + 7) / 8 + MD_MMA_WARPS - 1) / MD_MMA_WARPS;
             }
         }
         // tensors resident in shared memory: all of them when that is cheap, else a batch per row-block
@@ -88,12 +96,14 @@ cudaError_t mma_launch(const MmaCall &c, int nsm, cudaStream_t st, int *info) {
             const int per = std::max<long long>(1, (long long)(48 * 1024) / ((long long)rs * 8 * k.nkb));
             k.rslots = k.nkb * (int)std::min<long long>(per, c.Kket);
         }
-        const MmaSmem lay = mma_smem_layout(L, k.rslots, c.Kbra, c.Kket, 64 * MW, 8 * NW + 4);
+        const MmaSmem lay = mma_smem_layout(L, k.rslots, c.Kbra, c.Kket, 8 * MD_MMA_WARPS * MW, 8 * NW + 4);
         k.smem = (size_t)lay.total * 8;
         if (k.smem > (size_t)g_max_smem - 1024) continue;
-        k.ctas = k.smem <= (size_t)(g_max_smem + 1024) / 2 - 1024 ? 2 : 1;
+        k.warps = MD_MMA_WARPS;
+        k.ctas = (int)std::max<size_t>(1, std::min<size_t>(16 / MD_MMA_WARPS, (size_t)(g_max_smem + 1024) / (k.smem + 1024)));   // by shared memory and registers
+        if (MD_MMA_WARPS == 4 && k.ctas < 4) continue;
         // prefer two CTAs per SM unless one CTA saves more than a third of the warp-steps
-        auto score = [](const Cand &x) { return (double)x.cost * (x.ctas == 2 ? 1.0 : 1.35); };
+        auto score = [](const Cand &x) { return (double)x.cost * (x.ctas >= 2 ? 1.0 : 1.35); };
         // ties: fewer row blocks (each B fragment is reused by more row tiles), then the smaller tile
         const double d = score(k) - score(best);
         if (!have || d < -1e-9 || (d <= 1e-9 && k.nblocks < best.nblocks)) { best = k; have = true; }
@@ -108,7 +118,7 @@ cudaError_t mma_launch(const MmaCall &c, int nsm, cudaStream_t st, int *info) {
     g.s_q = c.s_q; g.s_bi = c.s_bi; g.s_ki = c.s_ki; g.s_ab = c.s_ab; g.s_cd = c.s_cd;
     g.boys_tab = c.boys_tab; g.rlut = c.rlut;
     const unsigned grid = (unsigned)std::min<long long>(c.nq, (long long)nsm * best.ctas);
-    g_fn[best.MW][NW]<<<grid, MD_MMA_THREADS, best.smem, st>>>(g);
+    g_fn[best.warps == 8][best.MW][NW]<<<grid, 32 * best.warps, best.smem, st>>>(g);
     if (info) {
         info[0] = best.MW; info[1] = NW; info[2] = (int)best.smem; info[3] = best.cached; info[4] = best.rslots;
         info[5] = best.nkb; info[6] = best.np; info[7] = best.ctas;
