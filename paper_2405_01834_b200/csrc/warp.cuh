@@ -93,25 +93,72 @@ __global__ void __launch_bounds__(MD_WARP_THREADS) eri_warp_kernel(WarpArgs g) {
                     __syncwarp();
                 }
                 // S4a: [p~|cd] (+)= sum_q~ [p~+q~]^(0) Hk[q~][cd]            (Eqs. 19, 25; the sign is in Hk)
+                // With enough Hermite rows the lanes own rows p~ and block 8 columns cd in registers: one gathered
+                // [p~+q~] feeds 8 FMAs and the Hk loads are warp-wide broadcasts; else one (p~, cd) element per lane.
                 const double *Hk = rk + 4;
-                for (int it = lane; it < nhb * g.ncd; it += 32) {
-                    const int p = it / g.ncd, cd = it - p * g.ncd;
-                    const uint32_t wp = s_w[p];
-                    double a = 0.0;
-                    for (int iq = g.kq0; iq < nhk; ++iq)
-                        a = fma(R0[herm_index_packed(wp + s_w[iq])], __ldg(Hk + (long long)iq * g.ncd + cd), a);
-                    if (kk == 0) half[it] = a; else half[it] += a;
+                if (nhb >= 16) {
+                    for (int cd0 = 0; cd0 < g.ncd; cd0 += 8) {
+                        const int nc = min(8, g.ncd - cd0);
+                        for (int p = lane; p < nhb; p += 32) {
+                            const uint32_t wp = s_w[p];
+                            double acc[8];
+#pragma unroll
+                            for (int c = 0; c < 8; ++c) acc[c] = 0.0;
+                            for (int iq = g.kq0; iq < nhk; ++iq) {
+                                const double r = R0[herm_index_packed(wp + s_w[iq])];
+                                const double *hk = Hk + (long long)iq * g.ncd + cd0;
+#pragma unroll
+                                for (int c = 0; c < 8; ++c)
+                                    if (c < nc) acc[c] = fma(r, __ldg(hk + c), acc[c]);
+                            }
+                            double *h = half + p * g.ncd + cd0;
+#pragma unroll
+                            for (int c = 0; c < 8; ++c)
+                                if (c < nc) { if (kk == 0) h[c] = acc[c]; else h[c] += acc[c]; }
+                        }
+                    }
+                } else {
+                    for (int it = lane; it < nhb * g.ncd; it += 32) {
+                        const int p = it / g.ncd, cd = it - p * g.ncd;
+                        const uint32_t wp = s_w[p];
+                        double a = 0.0;
+                        for (int iq = g.kq0; iq < nhk; ++iq)
+                            a = fma(R0[herm_index_packed(wp + s_w[iq])], __ldg(Hk + (long long)iq * g.ncd + cd), a);
+                        if (kk == 0) half[it] = a; else half[it] += a;
+                    }
                 }
             }
             __syncwarp();
             // S4b: [ab|cd] (+)= sum_p~ Hb[p~][ab] [p~|cd]                    (Eq. 26); S5 is folded into Hb, Hk
             const double *Hb = rb + 4;
-            for (int it = lane; it < g.nab * g.ncd; it += 32) {
-                const int ab = it / g.ncd, cd = it - ab * g.ncd;
-                double a = 0.0;
-                for (int p = 0; p < nhb; ++p) a = fma(__ldg(Hb + (long long)p * g.nab + ab), half[p * g.ncd + cd], a);
-                double *o = out + ab * g.s_ab + cd * g.s_cd;
-                if (kb == 0) *o = a; else *o += a;
+            if (g.nab >= 16) {                                  // lanes own ab, 8 columns cd in registers
+                for (int cd0 = 0; cd0 < g.ncd; cd0 += 8) {
+                    const int nc = min(8, g.ncd - cd0);
+                    for (int ab = lane; ab < g.nab; ab += 32) {
+                        double acc[8];
+#pragma unroll
+                        for (int c = 0; c < 8; ++c) acc[c] = 0.0;
+                        for (int p = 0; p < nhb; ++p) {
+                            const double hb = __ldg(Hb + (long long)p * g.nab + ab);
+                            const double *h = half + p * g.ncd + cd0;
+#pragma unroll
+                            for (int c = 0; c < 8; ++c)
+                                if (c < nc) acc[c] = fma(hb, h[c], acc[c]);
+                        }
+                        double *o = out + ab * g.s_ab + cd0 * g.s_cd;
+#pragma unroll
+                        for (int c = 0; c < 8; ++c)
+                            if (c < nc) { if (kb == 0) o[c * g.s_cd] = acc[c]; else o[c * g.s_cd] += acc[c]; }
+                    }
+                }
+            } else {
+                for (int it = lane; it < g.nab * g.ncd; it += 32) {
+                    const int ab = it / g.ncd, cd = it - ab * g.ncd;
+                    double a = 0.0;
+                    for (int p = 0; p < nhb; ++p) a = fma(__ldg(Hb + (long long)p * g.nab + ab), half[p * g.ncd + cd], a);
+                    double *o = out + ab * g.s_ab + cd * g.s_cd;
+                    if (kb == 0) *o = a; else *o += a;
+                }
             }
         }
     }
