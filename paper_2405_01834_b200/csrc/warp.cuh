@@ -96,7 +96,7 @@ __global__ void __launch_bounds__(MD_WARP_THREADS) eri_warp_kernel(WarpArgs g) {
                 // With enough Hermite rows the lanes own rows p~ and block 8 columns cd in registers: one gathered
                 // [p~+q~] feeds 8 FMAs and the Hk loads are warp-wide broadcasts; else one (p~, cd) element per lane.
                 const double *Hk = rk + 4;
-                if (nhb >= 16) {
+                if (nhb >= 16 && g.ncd >= 4) {
                     for (int cd0 = 0; cd0 < g.ncd; cd0 += 8) {
                         const int nc = min(8, g.ncd - cd0);
                         for (int p = lane; p < nhb; p += 32) {
@@ -131,7 +131,7 @@ __global__ void __launch_bounds__(MD_WARP_THREADS) eri_warp_kernel(WarpArgs g) {
             __syncwarp();
             // S4b: [ab|cd] (+)= sum_p~ Hb[p~][ab] [p~|cd]                    (Eq. 26); S5 is folded into Hb, Hk
             const double *Hb = rb + 4;
-            if (g.nab >= 16) {                                  // lanes own ab, 8 columns cd in registers
+            if (g.nab >= 16 && g.ncd >= 4) {                   // lanes own ab, 8 columns cd in registers
                 for (int cd0 = 0; cd0 < g.ncd; cd0 += 8) {
                     const int nc = min(8, g.ncd - cd0);
                     for (int ab = lane; ab < g.nab; ab += 32) {
