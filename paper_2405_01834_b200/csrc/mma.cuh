@@ -232,10 +232,42 @@ __global__ void __launch_bounds__(32 * MD_MMA_WARPS, 16 / MD_MMA_WARPS) eri_mma_
                     }
                 }
                 __syncthreads();
-                // GEMM2: units (ab tile, cd tile) round-robin over the warps, U2 units per warp per chunk
-                constexpr int U2 = 4;
-                const int nmt2 = (g.nab + 7) >> 3, nunits = nmt2 * nnt;
+                // GEMM2: a warp owns ab tiles (round-robin) and, for each, all cd tiles of the pass: one A fragment of
+                // Hb (global memory) feeds up to NW DMMAs, the B fragments come from [p~|cd] in shared memory.
+                const int nmt2 = (g.nab + 7) >> 3;
                 const int ksteps = (rows + 3) >> 2;
+                if (nmt2 >= 2 * MD_MMA_WARPS)
+                for (int um = warp; um < nmt2; um += MD_MMA_WARPS) {
+                    double c2[NW][2];
+#pragma unroll
+                    for (int n = 0; n < NW; ++n) c2[n][0] = c2[n][1] = 0.0;
+                    const int ab = um * 8 + lr;
+                    const bool abin = ab < g.nab;
+#pragma unroll 2
+                    for (int ks = 0; ks < ksteps; ++ks) {
+                        const int r = ks * 4 + lc;
+                        const int ro = rowoff[r];
+                        const double afr = (ro >= 0 && abin) ? __ldg(recb + ro + ab) : 0.0;
+                        const double *hrow = half + r * C::NTS + lr;
+#pragma unroll
+                        for (int n = 0; n < NW; ++n)
+                            if (n < nnt) dmma884(c2[n][0], c2[n][1], afr, hrow[n * 8]);
+                    }
+                    if (abin) {
+#pragma unroll
+                        for (int n = 0; n < NW; ++n) {
+                            if (n >= nnt) continue;
+                            const int cd = cd0 + n * 8 + 2 * lc;
+                            double *o = out + ab * g.s_ab + cd * g.s_cd;
+                            if (cd < g.ncd) { if (first) *o = c2[n][0]; else *o += c2[n][0]; }
+                            if (cd + 1 < g.ncd) { if (first) o[g.s_cd] = c2[n][1]; else o[g.s_cd] += c2[n][1]; }
+                        }
+                    }
+                }
+                else {
+                // few ab tiles: units (ab tile, cd tile) round-robin over the warps, U2 units per warp per chunk
+                constexpr int U2 = 4;
+                const int nunits = nmt2 * nnt;
                 for (int u0 = 0; u0 < nunits; u0 += U2 * MD_MMA_WARPS) {
                     double c2[U2][2];
                     int um[U2], un[U2];
@@ -270,6 +302,7 @@ __global__ void __launch_bounds__(32 * MD_MMA_WARPS, 16 / MD_MMA_WARPS) eri_mma_
                         if (cd < g.ncd) { if (first) *o = c2[i][0]; else *o += c2[i][0]; }
                         if (cd + 1 < g.ncd) { if (first) o[g.s_cd] = c2[i][1]; else o[g.s_cd] += c2[i][1]; }
                     }
+                }
                 }
                 first = false;
                 __syncthreads();                               // half / rowinfo are rewritten by the next row-block
