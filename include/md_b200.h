@@ -17,11 +17,20 @@
  *   output).  md_eri4_host / md_eri3_host take HOST pointers for every array and perform
  *   the host<->device copies themselves (they synchronise the stream before returning).
  *   The structs themselves are always host memory.  The caller owns every buffer; the
- *   library never frees or reallocates caller memory.  Scratch (per-pair Hermite data) is a
- *   grow-only device cache owned by the library unless md_set_workspace gives it a buffer.
+ *   library never frees or reallocates caller memory.  Scratch (per-pair Hermite data,
+ *   computed per call and never kept) is taken per call from the CUDA
+ *   stream-ordered memory pool on `cuda_stream` and returned to it after the call's last
+ *   kernel, unless md_set_workspace gives the library a caller-owned buffer.
  * Asynchrony.  md_eri4 / md_eri3 enqueue work on `cuda_stream` (a cudaStream_t cast to
- *   void*; NULL = the legacy default stream) and return without synchronising, as the
- *   paper's compute() does.  Growing the internal workspace synchronises.
+ *   void*; NULL = the legacy default stream) and return without any synchronisation, as the
+ *   paper's compute() does.  Calls in flight on different streams are
+ *   independent (each has its own scratch).  With a caller-owned workspace the caller must
+ *   order calls that share it (same stream, or events), as for any buffer it owns.
+ * Threads and devices.  One device per process: the first call binds the library to the
+ *   current device and calls made with another device current return MD_EINVAL.  md_init
+ *   is thread-safe; md_set_variant / md_set_workspace / md_last_* are process-wide
+ *   measurement and configuration state, so host threads that change them must serialise
+ *   their calls.
  * Errors.  Return 0 (MD_OK) or a negative code; nothing is written to `out` on an argument
  *   error.  No exception crosses the ABI.  md_last_cuda_error() returns the CUDA runtime's
  *   text for the most recent MD_ECUDA.
@@ -120,15 +129,21 @@ int md_eri3_host(const md_pairs *bra, const md_shells *X,
 int64_t md_eri4_out_elems(int la, int lb, int lc, int ld, int pure, int64_t nquartets);
 int64_t md_eri3_out_elems(int la, int lb, int lX, int pure, int64_t ntriplets);
 
-/* Scratch the library needs for a call with these shapes, in bytes (per-pair Hermite data,
- * PAPER.md:202 "{G, H[ab,p]}[ij,K_b]").  Classes served by a fused kernel need none. */
+/* Scratch, in bytes, that md_eri4 / md_eri3 would take for exactly this call (same batches,
+ * count, list_mode = quartet_idx != NULL, pure) with the kernel variant the library selects
+ * for it now (md_set_variant included): per-pair Hermite data (PAPER.md:202
+ * "{G, H[ab,p]}[ij,K_b]") or the per-CTA pair tables of the fused kernels; 0 if the kernel
+ * needs none.  A buffer of this size given to md_set_workspace is enough for that call.
+ * Only the struct fields are read (no device memory).  Negative error code on bad arguments. */
 int64_t md_eri4_workspace_bytes(const md_pairs *bra, const md_pairs *ket, int64_t nquartets,
                                 int list_mode, int pure);
 int64_t md_eri3_workspace_bytes(const md_pairs *bra, const md_shells *X, int64_t ntriplets,
                                 int list_mode, int pure);
 
-/* Give the library a caller-owned DEVICE scratch buffer (ptr == NULL returns to the internal
- * grow-only cache).  With a caller buffer a call that needs more returns MD_ENOMEM. */
+/* Give the library a caller-owned DEVICE scratch buffer (ptr == NULL returns to the
+ * stream-ordered pool).  With a caller buffer a call that needs more returns MD_ENOMEM before
+ * anything is launched or written (under MD_VARIANT_AUTO an l <= 2 class first falls back to
+ * the fused kernel that needs no scratch). */
 int md_set_workspace(void *device_ptr, size_t bytes);
 
 /* Kernel-variant control, for measurement:
@@ -159,7 +174,8 @@ int md_boys(int mmax, int scheme, int64_t n, const double *T, double *out, void 
 
 /* Measurement helper (not on the hot path): best achieved FP64 rate, in TFLOP/s, of a pure
  * issue loop running for about seconds_x10/10 s on the current device.
- *   kind 0: DFMA (vector pipe), 1: DMMA mma.sync.m8n8k4.f64, 2: DMMA mma.sync.m16n8k8.f64.
+ *   kind 0: DFMA (vector pipe), 1: DMMA mma.sync.m8n8k4.f64, 2: DMMA mma.sync.m16n8k8.f64,
+ *   3: DFMA and DMMA m8n8k4 issued by alternate warps of the same CTA (sum of both flop counts).
  * tflops and ms_out (duration of the best launch; may be NULL) are HOST pointers.  Synchronous. */
 int md_fp64_peak(int kind, int seconds_x10, double *tflops, double *ms_out);
 

@@ -37,7 +37,7 @@ cudaError_t fused2_init(int max_smem) {
 }
 
 int fused2_dispatch(const PairView &b0, const PairView &k0, long long nq, const int32_t *qidx, int pure, int layout,
-                    double *out, const double *boys_tab, int nsm, cudaStream_t st, int *info, int (*get_ws)(size_t, void **)) {
+                    double *out, const double *boys_tab, int nsm, cudaStream_t st, int *info, int (*get_ws)(void *, size_t, void **), void *ws_ctx) {
     if (b0.a.l > 2 || (!b0.single && b0.b.l > 2) || k0.a.l > 2 || (!k0.single && k0.b.l > 2)) return 0;
     Fused2Args ga;
     int l[4];
@@ -57,7 +57,7 @@ int fused2_dispatch(const PairView &b0, const PairView &k0, long long nq, const 
     const int Kbra = ga.f.bra.a.K * (ga.f.bra.single ? 1 : ga.f.bra.b.K), Kket = ga.f.ket.a.K * (ga.f.ket.single ? 1 : ga.f.ket.b.K);
     const size_t need = 8 * (size_t)grid * NQ * ((size_t)Kbra * e.brec + (size_t)Kket * e.krec);
     void *ws = nullptr;
-    int werr = get_ws(need, &ws);
+    int werr = get_ws(ws_ctx, need, &ws);
     if (werr) return werr;
     ga.scratch = (double *)ws;
     e.fn<<<grid, threads, smem, st>>>(ga);

@@ -15,9 +15,9 @@ int fused_dispatch(const PairView &b, const PairView &k, long long nq, const int
 
 // Warp-specialised fused kernels (fused2_inst.cu): same contract as fused_dispatch; info (may be null)
 // receives {PB, NCH, NQ, consumer threads, smem bytes}; get_ws supplies the per-CTA pair-table scratch
-// (returns < 0 with that error code if it cannot).
+// (a non-zero return value is passed back to the caller unchanged).
 cudaError_t fused2_init(int max_smem);
 int fused2_dispatch(const PairView &b, const PairView &k, long long nq, const int32_t *qidx, int pure, int layout,
-                    double *out, const double *boys_tab, int nsm, cudaStream_t st, int *info, int (*get_ws)(size_t, void **));
+                    double *out, const double *boys_tab, int nsm, cudaStream_t st, int *info, int (*get_ws)(void *, size_t, void **), void *ws_ctx);
 
 }  // namespace mdb

@@ -72,12 +72,19 @@ int host_call(const md_pairs *bra, const md_pairs *ket, const md_shells *X, int6
         CK(cudaStreamSynchronize(st));
         return MD_OK;
     }
-    static cudaStream_t copy_stream = nullptr;
-    static cudaEvent_t done[8];
-    if (!copy_stream) {
-        CK(cudaStreamCreateWithFlags(&copy_stream, cudaStreamNonBlocking));
-        for (auto &ev : done) CK(cudaEventCreateWithFlags(&ev, cudaEventDisableTiming));
-    }
+    // per-call copy stream and events (no state survives the call: the function is reentrant)
+    struct Copier {
+        cudaStream_t s = nullptr;
+        cudaEvent_t done[8] = {};
+        ~Copier() {
+            for (auto &ev : done) if (ev) cudaEventDestroy(ev);
+            if (s) cudaStreamDestroy(s);
+        }
+    } cp;
+    CK(cudaStreamCreateWithFlags(&cp.s, cudaStreamNonBlocking));
+    for (auto &ev : cp.done) CK(cudaEventCreateWithFlags(&ev, cudaEventDisableTiming));
+    cudaStream_t copy_stream = cp.s;
+    cudaEvent_t *done = cp.done;
     for (int c = 0; c < nchunk; ++c) {
         const int64_t q0 = n * c / nchunk, q1 = n * (c + 1) / nchunk, nc = q1 - q0;
         double *dchunk = (double *)dout + q0 * per;

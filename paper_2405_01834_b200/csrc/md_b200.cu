@@ -6,6 +6,7 @@
 #include <cmath>
 #include <cstdio>
 #include <cstring>
+#include <mutex>
 #include <vector>
 
 #include "../../include/md_b200.h"
@@ -26,8 +27,6 @@ struct State {
     bool init = false;
     int device = -1;
     double *boys_tab = nullptr;
-    void *ws = nullptr;          // internal grow-only workspace
-    size_t ws_bytes = 0;
     void *user_ws = nullptr;     // caller-owned workspace (md_set_workspace)
     size_t user_bytes = 0;
     int variant = MD_VARIANT_AUTO;
@@ -119,23 +118,39 @@ size_t generic_ws_bytes(const PairView &b, const PairView &k, int pure) {
     return 8 * ((size_t)b.npairs * s.Ka * s.Kb * s.stride_b + (size_t)k.npairs * s.Kc * s.Kd * s.stride_k);
 }
 
-int get_workspace(size_t bytes, void **out) {
-    if (S.user_ws) {
-        if (bytes > S.user_bytes) return MD_ENOMEM;
-        *out = S.user_ws;
+// Per-call scratch (pair data is computed per call and never kept).  Without a caller buffer the block is
+// taken from the CUDA stream-ordered pool on the call's own stream and released there after the last launch, so calls
+// in flight on different streams never share scratch and nothing synchronises.  In `dry` mode nothing is allocated or
+// launched: the first request records its size and the call unwinds with MD_DRY (the *_workspace_bytes queries).
+#define MD_DRY 2
+struct Scratch {
+    cudaStream_t st = nullptr;
+    void *owned = nullptr;
+    bool dry = false;
+    size_t need = 0;
+    int get(size_t bytes, void **out) {
+        need = bytes;
+        if (dry) return MD_DRY;
+        if (bytes == 0) { *out = nullptr; return MD_OK; }
+        if (S.user_ws) {
+            if (bytes > S.user_bytes) return MD_ENOMEM;
+            *out = S.user_ws;
+            return MD_OK;
+        }
+        CK(cudaMallocAsync(&owned, bytes, st));
+        *out = owned;
         return MD_OK;
     }
-    if (bytes > S.ws_bytes) {
-        CK(cudaDeviceSynchronize());                 // the old block may still be in use
-        if (S.ws) CK(cudaFree(S.ws));
-        S.ws = nullptr; S.ws_bytes = 0;
-        size_t want = bytes + bytes / 8 + (1 << 20);
-        CK(cudaMalloc(&S.ws, want));
-        S.ws_bytes = want;
+    void release() {
+        if (owned) cudaFreeAsync(owned, st);
+        owned = nullptr;
     }
-    *out = S.ws;
-    return MD_OK;
+};
+// Every class with all l <= 2 has a first-generation fused kernel (fused_inst.cu), which needs no scratch.
+bool fused_has_class(const PairView &b, const PairView &k) {
+    return b.a.l <= 2 && (b.single || b.b.l <= 2) && k.a.l <= 2 && (k.single || k.b.l <= 2);
 }
+int scratch_get(void *ctx, size_t bytes, void **out) { return ((Scratch *)ctx)->get(bytes, out); }
 
 int launch_pair_setup(const PairView &pv, int pure, int ket_sign, long long stride, double *rec, cudaStream_t st) {
     const int la = pv.a.l, lb = pv.single ? 0 : pv.b.l;
@@ -176,10 +191,10 @@ void out_strides(int layout, bool list_mode, long long nbra, long long nket, int
 }
 
 int run_generic(const PairView &b, const PairView &k, long long nq, const int32_t *qidx, int pure, int layout,
-                double *out, cudaStream_t st, bool use_mma) {
+                double *out, cudaStream_t st, bool use_mma, Scratch &sc) {
     Shape s = shape_of(b, k, pure);
     void *ws = nullptr;
-    int e = get_workspace(generic_ws_bytes(b, k, pure), &ws);
+    int e = sc.get(generic_ws_bytes(b, k, pure), &ws);
     if (e) return e;
     double *rec_b = (double *)ws;
     double *rec_k = rec_b + (size_t)b.npairs * s.Ka * s.Kb * s.stride_b;
@@ -228,10 +243,14 @@ int run_generic(const PairView &b, const PairView &k, long long nq, const int32_
         c.qidx = qidx; c.nq = nq; c.nket = k.npairs; c.out = out;
         c.s_q = g.s_q; c.s_bi = g.s_bi; c.s_ki = g.s_ki; c.s_ab = g.s_ab; c.s_cd = g.s_cd;
         c.boys_tab = S.boys_tab; c.rlut = fused_rlut();
-        CK(mma_launch(c, S.nsm, st, S.last_mma_info));
-        S.last_launches++;
-        S.last_variant = MD_VARIANT_MMA;
-        return MD_OK;
+        const cudaError_t me = mma_launch(c, S.nsm, st, S.last_mma_info);
+        if (me == cudaSuccess) {
+            S.last_launches++;
+            S.last_variant = MD_VARIANT_MMA;
+            return MD_OK;
+        }
+        if (me != cudaErrorInvalidConfiguration) return cuda_fail(me);
+        // no DMMA tile shape fits shared memory for this (class, K): the DFMA kernel below serves every class
     }
     unsigned grid = (unsigned)std::min<long long>(nq, (long long)S.nsm * 8);
     eri_generic_kernel<<<grid, MD_GEN_THREADS, smem, st>>>(g);
@@ -242,15 +261,15 @@ int run_generic(const PairView &b, const PairView &k, long long nq, const int32_
 }
 
 int run(const PairView &b, const PairView &k, long long nq, const int32_t *qidx, int pure, int layout,
-        double *out, long long cap, cudaStream_t st) {
+        double *out, long long cap, cudaStream_t st, Scratch &sc) {
     if (pure != 0 && pure != 1) return MD_EINVAL;
     if (layout != MD_LAYOUT_QUARTET_MAJOR && layout != MD_LAYOUT_PAPER) return MD_EINVAL;
     if (layout == MD_LAYOUT_PAPER && qidx) return MD_EINVAL;
     if (nq < 0) return MD_EINVAL;
     if (!qidx && nq != b.npairs * k.npairs) return MD_EINVAL;
     Shape s = shape_of(b, k, pure);
-    if ((long long)s.nab * s.ncd * nq > cap) return MD_ECAPACITY;
-    if (nq > 0 && !out) return MD_EINVAL;
+    if (!sc.dry && (long long)s.nab * s.ncd * nq > cap) return MD_ECAPACITY;
+    if (!sc.dry && nq > 0 && !out) return MD_EINVAL;
     int e = md_init();
     if (e) return e;
     S.last_launches = 0;
@@ -259,24 +278,27 @@ int run(const PairView &b, const PairView &k, long long nq, const int32_t *qidx,
     // setup over the whole ket list, and the one-warp-per-quartet kernel is then 2-3.5x faster than the fused one.
     const bool product_s_ket = S.variant == MD_VARIANT_AUTO && !qidx && k.a.l == 0 && (k.single || k.b.l == 0) &&
                                b.a.l + (b.single ? 0 : b.b.l) >= 4 && nq >= 8 * (b.npairs + k.npairs);
-    if (product_s_ket) return run_generic(b, k, nq, qidx, pure, layout, out, st, true);
+    if (product_s_ket) return run_generic(b, k, nq, qidx, pure, layout, out, st, true, sc);
     if (S.variant == MD_VARIANT_AUTO || S.variant == MD_VARIANT_FUSED2) {
         // By measurement (profiles/r01_sweep_l2.md): the warp-specialised kernel wins on every instantiated class
         // once the primitive loop is long enough to fill its pipeline, and on (dd|dd) for any K.
         const long long nprim = (long long)b.a.K * (b.single ? 1 : b.b.K) * k.a.K * (k.single ? 1 : k.b.K);
         const bool dddd = b.a.l == 2 && !b.single && b.b.l == 2 && k.a.l == 2 && !k.single && k.b.l == 2;
         if (S.variant == MD_VARIANT_FUSED2 || nprim >= 4 || (dddd && nq >= 150000)) {
-            int r = fused2_dispatch(b, k, nq, qidx, pure, layout, out, S.boys_tab, S.nsm, st, S.last_f2_info, get_workspace);
+            int r = fused2_dispatch(b, k, nq, qidx, pure, layout, out, S.boys_tab, S.nsm, st, S.last_f2_info, scratch_get, &sc);
             if (r == 1) {
                 S.last_launches++;
                 CK(cudaGetLastError());
                 S.last_variant = MD_VARIANT_FUSED2;
                 return MD_OK;
             }
-            if (r < 0) return r;
+            if (r == MD_DRY) return r;
+            // under AUTO a caller buffer too small for the pair tables falls through to the first fused kernel (no scratch)
+            if (r < 0 && !(r == MD_ENOMEM && S.variant == MD_VARIANT_AUTO)) return r;
         }
     }
     if (S.variant == MD_VARIANT_AUTO || S.variant == MD_VARIANT_FUSED || S.variant == MD_VARIANT_FUSED2) {
+        if (sc.dry && fused_has_class(b, k)) { sc.need = 0; return MD_DRY; }
         int r = fused_dispatch(b, k, nq, qidx, pure, layout, out, S.boys_tab, S.nsm, st, S.variant == MD_VARIANT_FUSED);
         if (r == 1) {
             S.last_launches++;
@@ -286,17 +308,43 @@ int run(const PairView &b, const PairView &k, long long nq, const int32_t *qidx,
         }
         if (r < 0) return r;
     }
-    return run_generic(b, k, nq, qidx, pure, layout, out, st, S.variant != MD_VARIANT_GENERIC);
+    return run_generic(b, k, nq, qidx, pure, layout, out, st, S.variant != MD_VARIANT_GENERIC, sc);
 }
+
+int run_call(const PairView &b, const PairView &k, long long nq, const int32_t *qidx, int pure, int layout,
+             double *out, long long cap, cudaStream_t st) {
+    Scratch sc;
+    sc.st = st;
+    const int e = run(b, k, nq, qidx, pure, layout, out, cap, st, sc);
+    sc.release();                                   // stream-ordered: after the kernels enqueued above
+    return e;
+}
+long long run_query(const PairView &b, const PairView &k, long long nq, int list_mode, int pure) {
+    Scratch sc;
+    sc.dry = true;
+    static const int32_t dummy[2] = {0, 0};        // only its non-NULL-ness is looked at in dry mode
+    const int e = run(b, k, nq, list_mode ? dummy : nullptr, pure, MD_LAYOUT_QUARTET_MAJOR, nullptr, 0, nullptr, sc);
+    if (e == MD_DRY) return (long long)sc.need;
+    return e < 0 ? e : 0;                           // MD_OK: nothing to do (nq == 0)
+}
+
 
 }  // namespace
 
 extern "C" {
 
 int md_init(void) {
+    static std::mutex mu;
+    std::lock_guard<std::mutex> lock(mu);
     int dev = 0;
     CK(cudaGetDevice(&dev));
-    if (S.init && S.device == dev) return MD_OK;
+    if (S.init) return S.device == dev ? MD_OK : MD_EINVAL;    // one device per process (include/md_b200.h)
+    {   // keep freed scratch in the stream-ordered pool instead of returning it to the driver at every synchronisation
+        cudaMemPool_t pool;
+        CK(cudaDeviceGetDefaultMemPool(&pool, dev));
+        uint64_t keep = ~0ull;
+        CK(cudaMemPoolSetAttribute(pool, cudaMemPoolAttrReleaseThreshold, &keep));
+    }
     std::vector<uint32_t> herm;
     std::vector<double> solid;
     make_tables(herm, solid);
@@ -306,7 +354,6 @@ int md_init(void) {
     inv[0] = 0.0;
     for (int m = 1; m < MD_LTOT + 8; ++m) inv[m] = 1.0 / (2 * m - 1);
     CK(cudaMemcpyToSymbol(c_inv_odd, inv, sizeof(inv)));
-    if (S.boys_tab) cudaFree(S.boys_tab);
     CK(cudaMalloc(&S.boys_tab, sizeof(double) * MD_BOYS_NROW * MD_BOYS_MTAB));
     boys_table_kernel<<<(MD_BOYS_NROW + 63) / 64, 64>>>(S.boys_tab);
     CK(cudaGetLastError());
@@ -335,8 +382,8 @@ int md_eri4(const md_pairs *bra, const md_pairs *ket, int64_t nquartets, const i
     int e = check_pairs(bra);
     if (e) return e;
     if ((e = check_pairs(ket))) return e;
-    return run(view(*bra), view(*ket), nquartets, quartet_idx, pure, layout, out, out_capacity_elems,
-               (cudaStream_t)cuda_stream);
+    return run_call(view(*bra), view(*ket), nquartets, quartet_idx, pure, layout, out, out_capacity_elems,
+                    (cudaStream_t)cuda_stream);
 }
 
 int md_eri3(const md_pairs *bra, const md_shells *X, int64_t ntriplets, const int32_t *triplet_idx, int pure,
@@ -344,8 +391,8 @@ int md_eri3(const md_pairs *bra, const md_shells *X, int64_t ntriplets, const in
     int e = check_pairs(bra);
     if (e) return e;
     if ((e = check_shells(X))) return e;
-    return run(view(*bra), view_single(*X), ntriplets, triplet_idx, pure, layout, out, out_capacity_elems,
-               (cudaStream_t)cuda_stream);
+    return run_call(view(*bra), view_single(*X), ntriplets, triplet_idx, pure, layout, out, out_capacity_elems,
+                    (cudaStream_t)cuda_stream);
 }
 
 int64_t md_eri4_out_elems(int la, int lb, int lc, int ld, int pure, int64_t n) {
@@ -359,14 +406,12 @@ int64_t md_eri3_out_elems(int la, int lb, int lX, int pure, int64_t n) {
 }
 
 int64_t md_eri4_workspace_bytes(const md_pairs *bra, const md_pairs *ket, int64_t nq, int list_mode, int pure) {
-    (void)nq; (void)list_mode;
     if (check_pairs(bra) || check_pairs(ket)) return MD_EINVAL;
-    return (int64_t)generic_ws_bytes(view(*bra), view(*ket), pure);
+    return run_query(view(*bra), view(*ket), nq, list_mode, pure);
 }
 int64_t md_eri3_workspace_bytes(const md_pairs *bra, const md_shells *X, int64_t nt, int list_mode, int pure) {
-    (void)nt; (void)list_mode;
     if (check_pairs(bra) || check_shells(X)) return MD_EINVAL;
-    return (int64_t)generic_ws_bytes(view(*bra), view_single(*X), pure);
+    return run_query(view(*bra), view_single(*X), nt, list_mode, pure);
 }
 
 int md_set_workspace(void *p, size_t bytes) {
@@ -393,7 +438,7 @@ int md_boys(int mmax, int scheme, int64_t n, const double *T, double *out, void 
 }
 
 int md_fp64_peak(int kind, int seconds_x10, double *tflops, double *ms_out) {
-    if (kind < 0 || kind > 2 || !tflops) return MD_EINVAL;
+    if (kind < 0 || kind > 3 || !tflops) return MD_EINVAL;
     int e = md_init();
     if (e) return e;
     double *d = nullptr;
@@ -405,14 +450,16 @@ int md_fp64_peak(int kind, int seconds_x10, double *tflops, double *ms_out) {
     int iters = 4096;
     double flop_per_iter = kind == 0 ? 2.0 * 16 * threads * blocks
                          : kind == 1 ? 512.0 * 8 * (threads / 32) * blocks
-                                     : 2048.0 * 4 * (threads / 32) * blocks;
+                         : kind == 2 ? 2048.0 * 4 * (threads / 32) * blocks
+                                     : (2.0 * 64 * 32 + 512.0 * 8) * (threads / 64) * blocks;
     double best = 0, total_ms = 0, ms_best = 0;
     const double budget_ms = 100.0 * (seconds_x10 > 0 ? seconds_x10 : 5);
     for (int rep = 0; rep < 1000 && total_ms < budget_ms; ++rep) {
         CK(cudaEventRecord(e0));
         if (kind == 0) peak_dfma_kernel<<<blocks, threads>>>(d, iters, 0.999999, 1e-9);
         else if (kind == 1) peak_dmma_kernel<<<blocks, threads>>>(d, iters, 0.999999, 1e-9);
-        else peak_dmma16_kernel<<<blocks, threads>>>(d, iters, 0.999999, 1e-9);
+        else if (kind == 2) peak_dmma16_kernel<<<blocks, threads>>>(d, iters, 0.999999, 1e-9);
+        else peak_mixed_kernel<<<blocks, threads>>>(d, iters, 0.999999, 1e-9);
         CK(cudaEventRecord(e1));
         CK(cudaEventSynchronize(e1));
         float ms = 0;

@@ -59,8 +59,10 @@ cudaError_t mma_launch(const MmaCall &c, int nsm, cudaStream_t st, int *info) {
     // with 4 warps); then the row-block shape.
     const bool small = nhb <= 128 && c.ncd <= 64;
     for (int MD_MMA_WARPS = small ? 4 : 8; MD_MMA_WARPS <= 8 && !have; MD_MMA_WARPS += 4)
-    for (int MW = 1; MW <= MWMAX; ++MW) {
+    for (int MW = 1; MW <= MWMAX; ++MW)
+    for (int shrink = 1; shrink <= 256; shrink *= 2) {          // halve the bra primitives per row block until it fits
         const int cap = 8 * MD_MMA_WARPS * MW;
+        if (shrink > 1 && (nhb > cap || shrink > c.Kbra)) break;
         Cand k{};
         k.MW = MW;
         if (nhb > cap) {
@@ -76,7 +78,7 @@ cudaError_t mma_launch(const MmaCall &c, int nsm, cudaStream_t st, int *info) {
             }
             k.cost *= c.Kbra;
         } else {
-            const int fit = std::min(c.Kbra, cap / nhb);
+            const int fit = std::max(1, std::min(c.Kbra, cap / nhb) / shrink);
             const int nblk = (c.Kbra + fit - 1) / fit;
             k.nkb = (c.Kbra + nblk - 1) / nblk;
             k.np = nhb;

@@ -56,4 +56,36 @@ __global__ void __launch_bounds__(256) peak_dmma16_kernel(double *out, int iters
     if (s == 12345.678) out[0] = s;
 }
 
+// Mixed: even warps run the DFMA chains, odd warps the m8n8k4 DMMA chains, same iteration count.  If the vector and
+// tensor FP64 paths were separate units the sum would exceed either peak; on B200 it does not.
+__global__ void __launch_bounds__(256) peak_mixed_kernel(double *out, int iters, double a, double b) {
+    double s = 0;
+    if ((threadIdx.x >> 5) & 1) {
+        double c[8][2];
+#pragma unroll
+        for (int i = 0; i < 8; ++i) { c[i][0] = threadIdx.x * 1e-3; c[i][1] = i; }
+        for (int it = 0; it < iters; ++it) {
+#pragma unroll
+            for (int i = 0; i < 8; ++i)
+                asm volatile("mma.sync.aligned.m8n8k4.row.col.f64.f64.f64.f64 {%0,%1}, {%2}, {%3}, {%0,%1};"
+                             : "+d"(c[i][0]), "+d"(c[i][1]) : "d"(a), "d"(b));
+        }
+#pragma unroll
+        for (int i = 0; i < 8; ++i) s += c[i][0] + c[i][1];
+    } else {
+        double x[16];
+#pragma unroll
+        for (int i = 0; i < 16; ++i) x[i] = threadIdx.x * 1e-3 + i;
+        for (int it = 0; it < iters; ++it) {            // 64 DFMA = the pipe time of the 8 DMMA above
+#pragma unroll
+            for (int r = 0; r < 4; ++r)
+#pragma unroll
+                for (int i = 0; i < 16; ++i) x[i] = fma(x[i], a, b);
+        }
+#pragma unroll
+        for (int i = 0; i < 16; ++i) s += x[i];
+    }
+    if (s == 12345.678) out[0] = s;
+}
+
 }  // namespace mdb

@@ -145,6 +145,26 @@ def md_set_variant(v):
     _check(lib().md_set_variant(int(v)))
 
 
+def md_set_workspace(buf):
+    """buf: a torch CUDA tensor used as caller-owned scratch, or None to return to the stream-ordered pool."""
+    if buf is None:
+        _check(lib().md_set_workspace(None, 0))
+    else:
+        _check(lib().md_set_workspace(_ptr(buf), buf.numel() * buf.element_size()))
+
+
+def md_eri4_workspace_bytes(a, b, c, d, bra_idx, ket_idx, nquartets, list_mode, pure, nbra=None, nket=None):
+    bra = _pairs_struct(a, b, bra_idx, nbra)
+    ket = _pairs_struct(c, d, ket_idx, nket)
+    return lib().md_eri4_workspace_bytes(ctypes.byref(bra), ctypes.byref(ket), int(nquartets), int(list_mode), int(pure))
+
+
+def md_eri3_workspace_bytes(a, b, x, bra_idx, ntriplets, list_mode, pure, nbra=None):
+    bra = _pairs_struct(a, b, bra_idx, nbra)
+    xs = _shells_struct(x)
+    return lib().md_eri3_workspace_bytes(ctypes.byref(bra), ctypes.byref(xs), int(ntriplets), int(list_mode), int(pure))
+
+
 def md_last_variant():
     return lib().md_last_variant()
 
@@ -231,6 +251,14 @@ class DeviceWorkload:
     def alloc_out(self, pure):
         import torch
         return torch.empty(self.w.nquartets * self.w.nout(pure), dtype=torch.float64, device=self.a.center.device)
+
+    def workspace_bytes(self, pure):
+        w = self.w
+        lm = w.quartet_idx is not None
+        if w.three_center:
+            return md_eri3_workspace_bytes(self.a, self.b, self.c, self.bra_idx, w.nquartets, lm, pure, nbra=w.nbra)
+        return md_eri4_workspace_bytes(self.a, self.b, self.c, self.d, self.bra_idx, self.ket_idx, w.nquartets, lm, pure,
+                                       nbra=w.nbra, nket=w.nket)
 
     def run(self, pure, out=None, layout=LAYOUT_QUARTET_MAJOR, stream=None):
         w = self.w

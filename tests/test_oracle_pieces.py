@@ -218,3 +218,25 @@ def test_solid_harmonics_are_harmonic_racah_normalised(l):
     assert abs(C[l, idx[(0, 0, l)]] - 1.0) < 1e-14                                    # S_l0(z^) = 1
     # rows are linearly independent (rank 2l+1)
     assert np.linalg.matrix_rank(C) == 2 * l + 1
+
+
+@pytest.mark.parametrize("l", range(7))
+def test_solid_harmonic_rows_vs_scipy(l):
+    """Order and sign of every row m = -l..l (the invariants above are blind to a row swap or sign
+    flip).  Library special case: with Y_lm = scipy's complex spherical harmonic (Condon-Shortley phase),
+    S_l0 = c r^l Y_l0,  S_l,+m = c r^l sqrt2 (-1)^m Re Y_lm,  S_l,-m = c r^l sqrt2 (-1)^m Im Y_lm,  c = sqrt(4 pi/(2l+1)):
+    the Racah-normalised real solid harmonics without the phase (reading O2/S2)."""
+    from scipy.special import sph_harm_y
+    C = oracle.cart2solid(l)
+    comps = [(ax, ay, l - ax - ay) for ax in range(l, -1, -1) for ay in range(l - ax, -1, -1)]
+    rng = np.random.default_rng(100 + l)
+    xyz = rng.normal(size=(12, 3))
+    r = np.linalg.norm(xyz, axis=1)
+    theta, phi = np.arccos(xyz[:, 2] / r), np.arctan2(xyz[:, 1], xyz[:, 0])
+    mono = np.array([[np.prod(v ** np.array(c)) for c in comps] for v in xyz])
+    S = mono @ C.T                                                   # [point][m + l]
+    c = math.sqrt(4 * math.pi / (2 * l + 1)) * r ** l
+    for m in range(-l, l + 1):
+        Y = sph_harm_y(l, abs(m), theta, phi)
+        ref = c * Y.real if m == 0 else c * math.sqrt(2) * (-1) ** m * (Y.real if m > 0 else Y.imag)
+        assert np.allclose(S[:, m + l], ref, rtol=1e-12, atol=1e-13), (l, m)
