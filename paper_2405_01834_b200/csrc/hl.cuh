@@ -1,0 +1,513 @@
+// hl.cuh -- the high-l quartet kernel: steps S1-S5 in ONE launch for classes with an l >= 3 shell.
+//
+// One persistent CTA evaluates one quartet (or triplet) at a time:
+//   S1  per primitive pair of both sides: the three 1-D Hermite tables (Eqs. 9, 10, 13, 14) by a warp
+//       per Cartesian axis, then the dense Hermite->AO matrices H (Eq. 17: solid harmonics folded in, ket sign
+//       of Eq. 19 folded in) by all threads, register-blocked, one index at a time.  The matrices go to a
+//       PER-CTA scratch in global memory (L2), never to a per-pair workspace: the scratch of the whole grid is a
+//       few hundred MB whatever the number of quartets (no N_shells^2 data is stored);
+//   S2-S3  Boys function and the Hermite Coulomb tensors [r~]^(0) of all primitive quartets, level by level
+//       (Eqs. 21-24), in shared memory;
+//   S4  per cd tile of NT = 8 NW columns, both contractions on the FP64 tensor path (mma.sync.m8n8k4.f64):
+//         GEMM1  [p~|cd] = sum_kk sum_q~ [p~+q~]^(0) Hk(kk)[q~][cd]   (Eqs. 19, 25), A gathered from the tensor,
+//         GEMM2  [ab|cd] = sum_(kb,p~) Hb(kb)[p~][ab] [p~|cd]          (Eq. 26),
+//       with BOTH H operands streamed from the scratch into a shared-memory ring by cp.async.bulk (TMA bulk
+//       copies) completing on mbarriers, a few chunks ahead of the tensor-core loop;
+//   S5  the accumulators of GEMM2 are the final [ab|cd] tile: stored once, no read-modify-write.
+// tcgen05 has no FP64 kind, so mma.sync is the only tensor path FP64 has on sm_100a.
+#pragma once
+#include "boys.cuh"
+#include "common.cuh"
+
+namespace mdb {
+
+#define MD_HL_KC1 32          // ket Hermite rows per ring chunk of GEMM1
+#define MD_HL_KC2 8           // stacked bra rows per ring chunk of GEMM2
+#define MD_HL_STAGES 4
+#define MD_HL_MT2 3           // ab row tiles per warp in GEMM2 (register-resident output)
+#define MD_HL_CSTR 14         // row stride of the transposed Cartesian->solid tables [cart][m], 13 padded to 14
+
+struct HlArgs {
+    PairView bra, ket;
+    int pure;
+    int la, lb, lc, ld;                  // ld = 0 for a one-centre ket
+    int Ka, Kb, Kc, Kd, Kbra, Kket;
+    int Lb, Lk, nab, ncd, nhb, nhk;
+    int mrows, mrows_pad;                // stacked rows (kb, p~) of [p~|cd]; padded to a multiple of 8
+    int nhk_pad;                         // ket Hermite rows padded to MD_HL_KC1
+    int sb;                              // row stride of Hb in the scratch: >= 8*ceil(nab/8), = 4 mod 16
+    int ntile;                           // cd tiles
+    int q_first;                         // first GEMM1 chunk row with a non-zero Hk (one-centre solid kets), multiple of KC1
+    double *scratch;                     // [grid][scratch_stride]
+    long long scratch_stride, off_hk;    // doubles per CTA; offset of the ket part
+    const int32_t *qidx;
+    long long nq, nket;
+    double *out;
+    long long s_q, s_bi, s_ki, s_ab, s_cd;
+    const double *boys_tab;
+    const uint32_t *rlut;
+    // shared-memory carve-up (doubles from the base)
+    int o_herm, o_rowinfo, o_ct, o_hdr, o_bar, o_r0, o_g0, o_pq, o_ov, o_ring, total;
+    int rs0, rs1, ov_doubles, ring_stage;
+};
+
+// ---- mbarrier / bulk-copy primitives (PTX ISA: mbarrier, cp.async.bulk) -------------------------------------------
+__device__ __forceinline__ uint32_t hl_saddr(const void *p) { return (uint32_t)__cvta_generic_to_shared(p); }
+__device__ __forceinline__ void hl_bar_init(uint64_t *b, int count) {
+    asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(hl_saddr(b)), "r"(count));
+}
+__device__ __forceinline__ void hl_bar_expect(uint64_t *b, uint32_t bytes) {
+    asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(hl_saddr(b)), "r"(bytes) : "memory");
+}
+__device__ __forceinline__ void hl_bar_arrive(uint64_t *b) {
+    asm volatile("mbarrier.arrive.shared::cta.b64 _, [%0];" ::"r"(hl_saddr(b)) : "memory");
+}
+__device__ __forceinline__ void hl_bar_wait(uint64_t *b, uint32_t parity) {
+    asm volatile(
+        "{\n .reg .pred p;\n WAIT_%=:\n mbarrier.try_wait.parity.shared::cta.b64 p, [%0], %1;\n @p bra DONE_%=;\n bra WAIT_%=;\n DONE_%=:\n}"
+        ::"r"(hl_saddr(b)), "r"(parity) : "memory");
+}
+__device__ __forceinline__ void hl_bulk_g2s(void *dst, const void *src, uint32_t bytes, uint64_t *b) {
+    asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];"
+                 ::"r"(hl_saddr(dst)), "l"(src), "r"(bytes), "r"(hl_saddr(b)) : "memory");
+}
+
+__device__ __forceinline__ void hl_dmma884(double &c0, double &c1, double a, double b) {
+    asm("mma.sync.aligned.m8n8k4.row.col.f64.f64.f64.f64 {%0,%1}, {%2}, {%3}, {%0,%1};"
+        : "+d"(c0), "+d"(c1) : "d"(a), "d"(b));
+}
+
+// Compact index of the Hermite triple with packed word w = t | u<<8 | v<<16 | n<<24 (degree-sorted list, common.cuh).
+__device__ __forceinline__ int hl_herm_index(uint32_t w) {
+    const int n = w >> 24, t = w & 0xff, v = (w >> 16) & 0xff, a = n - t;
+    return ((n * (n + 1) * (n + 2) * 10923) >> 16) + ((a * (a + 1)) >> 1) + v;
+}
+
+// ---- S1: one Cartesian axis of the two-centre Hermite expansion, by one warp (lane = t) -----------------------------
+//   E^0_00 = exp(-za zb xab^2/p)                                              (Eq. 13)
+//   E^t_{i,j+1} = E^{t-1}_{ij}/(2p) + (P-B) E^t_{ij} + (t+1) E^{t+1}_{ij}     (Eq. 10), along i = 0
+//   E^t_{i+1,j} = E^{t-1}_{ij}/(2p) + (P-A) E^t_{ij} + (t+1) E^{t+1}_{ij}     (Eq. 9),  for every j
+// E[(i*(lb+1)+j)*nt + t], nt = la+lb+1 <= 13; entries with t > i+j are written as exact zeros (Eq. 14), which the
+// H build relies on.  A one-centre expansion (Eq. 8) is the case zb = 0, xab = 0.
+__device__ __forceinline__ void hl_e_axis_warp(int la, int lb, double za, double zb, double xab, double *E, int lane) {
+    const int nt = la + lb + 1;
+    const double p = za + zb, h = 0.5 / p;
+    const double xpa = -zb * xab / p, xpb = za * xab / p;
+    const double tp1 = (double)(lane + 1);
+    double e = lane == 0 ? exp(-za * zb / p * xab * xab) : 0.0;
+    if (lane < nt) E[lane] = e;
+    for (int j = 0; j < lb; ++j) {
+        double em = __shfl_up_sync(0xffffffffu, e, 1), ep = __shfl_down_sync(0xffffffffu, e, 1);
+        if (lane == 0) em = 0.0;
+        if (lane == 31) ep = 0.0;
+        e = xpb * e + h * em + tp1 * ep;
+        if (lane < nt) E[(j + 1) * nt + lane] = e;
+    }
+    for (int j = 0; j <= lb; ++j) {
+        e = lane < nt ? E[j * nt + lane] : 0.0;
+        for (int i = 0; i < la; ++i) {
+            double em = __shfl_up_sync(0xffffffffu, e, 1), ep = __shfl_down_sync(0xffffffffu, e, 1);
+            if (lane == 0) em = 0.0;
+            if (lane == 31) ep = 0.0;
+            e = xpa * e + h * em + tp1 * ep;
+            if (lane < nt) E[((i + 1) * (lb + 1) + j) * nt + lane] = e;
+        }
+    }
+}
+
+// Where H[p~][m] of one primitive pair goes in the CTA's scratch.
+struct HlBraDst {            // [kb*nhb + p~][sb]
+    double *base; int sb;
+    __device__ __forceinline__ double *operator()(int p, int m) const { return base + (long long)p * sb + m; }
+};
+template <int NT>
+struct HlKetDst {            // tile-major: [cd tile][kk][q~ (padded)][NT + 4]
+    double *base; long long tile_stride;     // Kket * nhk_pad * (NT+4)
+    __device__ __forceinline__ double *operator()(int q, int m) const {
+        const int j = m / NT, n = m - j * NT;
+        return base + j * tile_stride + (long long)q * (NT + 4) + n;
+    }
+};
+
+// ---- S1: dense H of one primitive pair (Eqs. 7, 17), all threads of the CTA ---------------------------------
+//   Cartesian: H[p~][ab]   = c E^t_{ax bx} E^u_{ay by} E^v_{az bz}
+//   solid    : H[p~][mamb] = c sum_a C^{la}_{ma,a} sum_b C^{lb}_{mb,b} E^{ab}_{p~}, one index at a time:
+//     stage A  task (p~, a):  T1[p~][a][mb] = sum_b C^{lb}[mb][b] E^{ab}_{p~}   (13 accumulators in registers)
+//     stage B  task (p~, mb): H[p~][ma][mb] = c sum_a C^{la}[ma][a] T1[p~][a][mb]
+//   Steps whose operand is zero for the whole warp are skipped (Eq. 14 makes 80 % of E^{ab}_{p~} vanish).
+// E = the three axis tables (shared memory), T1 = shared scratch of t1cap doubles, CaT/CbT = transposed
+// Cartesian->solid tables [cart][MD_HL_CSTR].  Ends with a barrier.  neg: fold (-1)^{|q~|} (Eq. 19).
+template <int NTHR, class Dst>
+__device__ __forceinline__ void hl_build_H(int la, int lb, int pure, bool neg, double coef, const double *E, double *T1,
+                                           int t1cap, const uint32_t *s_herm, const double *CaT, const double *CbT,
+                                           const Dst &dst) {
+    const int tid = threadIdx.x;
+    const int Lb = la + lb, nt = Lb + 1, nh = nherm(Lb), esz = (la + 1) * (lb + 1) * nt;
+    const int nca = ncart(la), ncb = ncart(lb);
+    const uint32_t *ca = s_herm + nherm(la - 1), *cb = s_herm + nherm(lb - 1);
+    const double *Ex = E, *Ey = E + esz, *Ez = E + 2 * esz;
+    if (!pure) {
+        const int nab = nca * ncb;
+        for (int e = tid; e < nh * nab; e += NTHR) {
+            const int ih = e / nab, ab = e - ih * nab, a = ab / ncb, b = ab - a * ncb;
+            int t, u, v, ax, ay, az, bx, by, bz;
+            unpack_tuv(s_herm[ih], t, u, v);
+            unpack_tuv(ca[a], ax, ay, az);
+            unpack_tuv(cb[b], bx, by, bz);
+            double val = coef * Ex[(ax * (lb + 1) + bx) * nt + t] * Ey[(ay * (lb + 1) + by) * nt + u] *
+                         Ez[(az * (lb + 1) + bz) * nt + v];
+            if (neg && ((t + u + v) & 1)) val = -val;
+            *dst(ih, ab) = val;
+        }
+        __syncthreads();
+        return;
+    }
+    const int nsa = nsolid(la), nsb = nsolid(lb);
+    const int pchunk = max(1, min(nh, t1cap / (nca * nsb)));
+    for (int h0 = 0; h0 < nh; h0 += pchunk) {
+        const int hc = min(pchunk, nh - h0);
+        for (int e = tid; e < hc * nca; e += NTHR) {
+            const int ih = e / nca, a = e - ih * nca;
+            int t, u, v, ax, ay, az;
+            unpack_tuv(s_herm[h0 + ih], t, u, v);
+            unpack_tuv(ca[a], ax, ay, az);
+            const double *ex = Ex + ax * (lb + 1) * nt + t, *ey = Ey + ay * (lb + 1) * nt + u, *ez = Ez + az * (lb + 1) * nt + v;
+            double acc[13];
+#pragma unroll
+            for (int m = 0; m < 13; ++m) acc[m] = 0.0;
+            for (int b = 0; b < ncb; ++b) {
+                int bx, by, bz;
+                unpack_tuv(cb[b], bx, by, bz);
+                const double x = ex[bx * nt] * ey[by * nt] * ez[bz * nt];
+                if (!__any_sync(__activemask(), x != 0.0)) continue;
+                const double *c = CbT + b * MD_HL_CSTR;
+#pragma unroll
+                for (int m = 0; m < 13; ++m)
+                    if (m < nsb) acc[m] = fma(c[m], x, acc[m]);
+            }
+            double *o = T1 + (size_t)e * nsb;
+#pragma unroll
+            for (int m = 0; m < 13; ++m)
+                if (m < nsb) o[m] = acc[m];
+        }
+        __syncthreads();
+        for (int e = tid; e < hc * nsb; e += NTHR) {
+            const int ih = e / nsb, mb = e - ih * nsb;
+            const double *t1 = T1 + (size_t)ih * nca * nsb + mb;
+            double acc[13];
+#pragma unroll
+            for (int m = 0; m < 13; ++m) acc[m] = 0.0;
+            for (int a = 0; a < nca; ++a) {
+                const double y = t1[a * nsb];
+                if (!__any_sync(__activemask(), y != 0.0)) continue;
+                const double *c = CaT + a * MD_HL_CSTR;
+#pragma unroll
+                for (int m = 0; m < 13; ++m)
+                    if (m < nsa) acc[m] = fma(c[m], y, acc[m]);
+            }
+            const double s = (neg && (s_herm[h0 + ih] >> 24 & 1)) ? -coef : coef;
+#pragma unroll
+            for (int m = 0; m < 13; ++m)
+                if (m < nsa) *dst(h0 + ih, m * nsb + mb) = s * acc[m];
+        }
+        __syncthreads();
+    }
+}
+
+// Order in which one quartet's H chunks pass through the ring: for every cd tile, for every row pass of GEMM1 the
+// chunks (kk, c) of Hk, then the chunks of Hb for GEMM2.  Only the producer thread advances it.
+struct HlStream {
+    int j, pass, kk, c, c2;
+    __device__ __forceinline__ void reset(int c_first) { j = 0; pass = 0; kk = 0; c = c_first; c2 = -1; }
+};
+
+template <int MW, int NW, int NWARPS>
+__global__ void __launch_bounds__(32 * NWARPS, (NWARPS == 4 ? 3 : (MW <= 2 ? 2 : 1))) hl_kernel(HlArgs g) {
+    constexpr int NTHR = 32 * NWARPS, NT = 8 * NW, NTS = NT + 4, ST = MD_HL_STAGES;
+    extern __shared__ double sm[];
+    uint32_t *s_herm = (uint32_t *)(sm + g.o_herm);
+    int2 *rowinfo = (int2 *)(sm + g.o_rowinfo);            // .x = packed (t,u,v,n) of p~, .y = kb
+    double *CT = sm + g.o_ct;                              // 4 transposed Cartesian->solid tables
+    double *hdr = sm + g.o_hdr;                            // {p, Px, Py, Pz} per bra primitive, then per ket primitive
+    uint64_t *full = (uint64_t *)(sm + g.o_bar), *empty = full + ST;
+    double *R0 = sm + g.o_r0, *G0 = sm + g.o_g0, *PQ = sm + g.o_pq;
+    double *ov = sm + g.o_ov;                              // [p~|cd] tile; before that R1 / the S1 scratch (spans the ring too)
+    double *R1 = ov, *Vp = ov;
+    double *ring = sm + g.o_ring;
+    const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+    const int lr = lane >> 2, lc = lane & 3;
+    const int L = g.Lb + g.Lk, nhb = g.nhb, nhk = g.nhk;
+    const uint2 *lut = (const uint2 *)g.rlut;
+    const int CTS = 28 * MD_HL_CSTR;
+    double *scr = g.scratch + (long long)blockIdx.x * g.scratch_stride;
+    double *hb = scr, *hk = scr + g.off_hk;
+    const int nmt = g.mrows_pad >> 3, npass = (nmt + NWARPS * MW - 1) / (NWARPS * MW);
+    const int nc1 = g.nhk_pad / MD_HL_KC1, c_first = g.q_first / MD_HL_KC1, nc2 = g.mrows_pad / MD_HL_KC2;
+    const int nmt2 = (g.nab + 7) >> 3;
+    const long long hk_tile = (long long)g.Kket * g.nhk_pad * NTS;
+    const uint32_t bytes1 = MD_HL_KC1 * NTS * 8, bytes2 = MD_HL_KC2 * g.sb * 8;
+
+    // ---- once per CTA: constant tables, barriers, zeroed scratch (its padding is never written again) ----
+    {
+        const int nhm = nherm(max(g.Lb, g.Lk));
+        for (int i = tid; i < nhm; i += NTHR) s_herm[i] = c_herm[i];
+        const int ls[4] = {g.la, g.lb, g.lc, g.ld};
+        for (int s = 0; s < 4; ++s) {
+            const int l = ls[s], nc = ncart(l), ns = nsolid(l);
+            for (int i = tid; i < nc * ns; i += NTHR) {
+                const int m = i / nc, c = i - m * nc;
+                CT[s * CTS + c * MD_HL_CSTR + m] = c_solid[solid_off(l) + i];
+            }
+        }
+        for (int r = tid; r < g.mrows_pad; r += NTHR) {
+            const int rr = min(r, g.mrows - 1), kb = rr / nhb;
+            rowinfo[r] = make_int2((int)c_herm[rr - kb * nhb], kb);
+        }
+        if (tid == 0) {
+            for (int s = 0; s < ST; ++s) { hl_bar_init(full + s, 1); hl_bar_init(empty + s, NWARPS); }
+            asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+        }
+        for (long long i = tid; i < g.scratch_stride; i += NTHR) scr[i] = 0.0;
+    }
+    long long gcons = 0, gprod = 0;                        // chunks consumed (all threads) / issued (thread 0), CTA lifetime
+    HlStream ps;
+    long long left = 0;                                    // chunks of the current quartet not yet issued (thread 0)
+    const long long per_quartet = (long long)g.ntile * ((long long)npass * g.Kket * (nc1 - c_first) + nc2);
+
+    auto produce = [&]() {                                 // thread 0: issue the next chunk of the stream
+        const int s = (int)(gprod % ST);
+        if (gprod >= ST) hl_bar_wait(empty + s, (uint32_t)((gprod / ST - 1) & 1));
+        const double *src;
+        uint32_t bytes;
+        if (ps.c2 < 0) {
+            src = hk + ps.j * hk_tile + ((long long)ps.kk * g.nhk_pad + (long long)ps.c * MD_HL_KC1) * NTS;
+            bytes = bytes1;
+            if (++ps.c == nc1) { ps.c = c_first; if (++ps.kk == g.Kket) { ps.kk = 0; if (++ps.pass == npass) { ps.pass = 0; ps.c2 = 0; } } }
+        } else {
+            src = hb + (long long)ps.c2 * MD_HL_KC2 * g.sb;
+            bytes = bytes2;
+            if (++ps.c2 == nc2) { ps.c2 = -1; ++ps.j; }
+        }
+        hl_bar_expect(full + s, bytes);
+        hl_bulk_g2s(ring + (size_t)s * g.ring_stage, src, bytes, full + s);
+        ++gprod; --left;
+    };
+    auto acquire = [&]() -> const double * {               // all threads: wait for the next chunk
+        const int s = (int)(gcons % ST);
+        hl_bar_wait(full + s, (uint32_t)((gcons / ST) & 1));
+        return ring + (size_t)s * g.ring_stage;
+    };
+    auto release = [&]() {                                 // all threads: done with it; thread 0 tops the ring up
+        __syncwarp();
+        if (lane == 0) hl_bar_arrive(empty + (int)(gcons % ST));
+        ++gcons;
+        if (tid == 0 && left > 0) produce();
+    };
+
+    for (long long q = blockIdx.x; q < g.nq; q += gridDim.x) {
+        long long bi, ki;
+        if (g.qidx) { bi = g.qidx[2 * q]; ki = g.qidx[2 * q + 1]; }
+        else { bi = q / g.nket; ki = q % g.nket; }
+        double *out = g.out + q * g.s_q + bi * g.s_bi + ki * g.s_ki;
+        __syncthreads();                                   // the previous quartet is done with shared memory and the scratch
+
+        // ---- S1: Hermite tables and H of every primitive pair of both sides -> scratch ----
+        for (int side = 0; side < 2; ++side) {
+            const PairView &pv = side ? g.ket : g.bra;
+            const int l1 = side ? g.lc : g.la, l2 = side ? g.ld : g.lb;
+            const int K1 = side ? g.Kc : g.Ka, K2 = side ? g.Kd : g.Kb;
+            const long long ip = side ? ki : bi;
+            long long i1 = ip, i2 = ip;
+            if (pv.idx) { i1 = pv.idx[2 * ip]; i2 = pv.idx[2 * ip + 1]; }
+            const int esz = (l1 + 1) * (l2 + 1) * (l1 + l2 + 1);
+            double *E = ov, *T1 = ov + 3 * esz;
+            const int t1cap = g.ov_doubles + ST * g.ring_stage - 3 * esz;
+            for (int kp = 0; kp < K1 * K2; ++kp) {
+                const int k1 = kp / K2, k2 = kp - k1 * K2;
+                const double za = pv.a.exps[i1 * K1 + k1];
+                const double zb = pv.single ? 0.0 : pv.b.exps[i2 * K2 + k2];
+                const double coef = pv.a.coefs[i1 * K1 + k1] * (pv.single ? 1.0 : pv.b.coefs[i2 * K2 + k2]);
+                if (warp < 3) {
+                    const double A = pv.a.center[3 * i1 + warp], B = pv.single ? A : pv.b.center[3 * i2 + warp];
+                    hl_e_axis_warp(l1, l2, za, zb, A - B, E + warp * esz, lane);
+                    if (lane == 0) {
+                        double *h = hdr + 4 * ((side ? g.Kbra : 0) + kp);
+                        h[1 + warp] = (za * A + zb * B) / (za + zb);
+                        if (warp == 0) h[0] = za + zb;
+                    }
+                }
+                __syncthreads();
+                const double *CaT = CT + (side ? 2 : 0) * CTS, *CbT = CT + (side ? 3 : 1) * CTS;
+                if (pv.single && g.pure) {
+                    // One-centre solid harmonics (Hobson): S_lm(d/dA) e^{-z r_A^2} = (2z)^l S_lm(r_A) e^{-z r_A^2}: only the
+                    // Hermites of order exactly l appear, with coefficient C^l_{m,q~}/(2z)^l; lower rows are exact zeros.
+                    const int ns = nsolid(l1), nlow = nherm(l1 - 1);
+                    double f = coef;
+                    for (int i = 0; i < l1; ++i) f *= 0.5 / za;
+                    if (l1 & 1) f = -f;
+                    HlKetDst<NT> dst{hk + (long long)kp * g.nhk_pad * NTS, hk_tile};
+                    for (int e = tid; e < nhk * ns; e += NTHR) {
+                        const int ih = e / ns, m = e - ih * ns;
+                        *dst(ih, m) = ih < nlow ? 0.0 : f * CaT[(ih - nlow) * MD_HL_CSTR + m];
+                    }
+                    __syncthreads();
+                } else if (side) {
+                    HlKetDst<NT> dst{hk + (long long)kp * g.nhk_pad * NTS, hk_tile};
+                    hl_build_H<NTHR>(l1, l2, g.pure, true, coef, E, T1, t1cap, s_herm, CaT, CbT, dst);
+                } else {
+                    HlBraDst dst{hb + (long long)kp * nhb * g.sb, g.sb};
+                    hl_build_H<NTHR>(l1, l2, g.pure, false, coef, E, T1, t1cap, s_herm, CaT, CbT, dst);
+                }
+            }
+        }
+        __threadfence();
+        asm volatile("fence.proxy.async;" ::: "memory");   // generic-proxy stores to the scratch before the bulk copies read it
+        __syncthreads();
+        if (tid == 0) {
+            ps.reset(c_first);
+            left = per_quartet;
+            for (int i = 0; i < ST - 1 && left > 0; ++i) produce();
+        }
+
+        // ---- S2-S3: [0]^(m) (Eq. 21) and Eq. 24 level by level for every primitive quartet; slot = kk*Kbra + kb ----
+        {
+            const int nR = g.Kbra * g.Kket;
+            for (int it = tid; it < nR * (L + 1); it += NTHR) {
+                const int s = it / (L + 1), m = it - s * (L + 1);
+                const double *hbp = hdr + 4 * (s % g.Kbra), *hkp = hdr + 4 * (g.Kbra + s / g.Kbra);
+                const double p = hbp[0], qq = hkp[0];
+                const double X = hbp[1] - hkp[1], Y = hbp[2] - hkp[2], Z = hbp[3] - hkp[3];
+                const double rho = p * qq / (p + qq);
+                const double T = rho * (X * X + Y * Y + Z * Z);
+                double f = 34.98683665524972497 / (p * qq * sqrt(p + qq)) * boys_single(m, T, g.boys_tab);   // 2 pi^{5/2}
+                const double m2r = -2.0 * rho;
+                for (int i = 0; i < m; ++i) f *= m2r;
+                G0[s * (L + 1) + m] = f;
+                if (m == L) ((L & 1) ? R1 + s * g.rs1 : R0 + s * g.rs0)[0] = f;
+                if (m == 0) { PQ[3 * s] = X; PQ[3 * s + 1] = Y; PQ[3 * s + 2] = Z; }
+            }
+            __syncthreads();
+            for (int m = L - 1; m >= 0; --m) {
+                const int ne = nherm(L - m);
+                for (int s = warp; s < nR; s += NWARPS) {
+                    const double *old = (m & 1) ? R0 + s * g.rs0 : R1 + s * g.rs1;
+                    double *nw = (m & 1) ? R1 + s * g.rs1 : R0 + s * g.rs0;
+                    const double *pq = PQ + 3 * s;
+                    for (int e = lane; e < ne; e += 32) {
+                        const uint32_t w = __ldg(&lut[e].x);
+                        double val;
+                        if (e == 0) val = G0[s * (L + 1) + m];
+                        else {
+                            val = pq[w >> 24 & 3] * old[w & 0xfff];
+                            const int cf = w >> 26;
+                            if (cf) val = fma((double)cf, old[w >> 12 & 0xfff], val);
+                        }
+                        nw[e] = val;
+                    }
+                }
+                __syncthreads();
+            }
+        }
+
+        // ---- S4-S5 per cd tile ----
+        for (int j = 0; j < g.ntile; ++j) {
+            const int cd0 = j * NT;
+            const int nnt = min(NW, (g.ncd - cd0 + 7) >> 3);
+            // GEMM1 (Eqs. 19, 25): rows = stacked (kb, p~), columns = this cd tile, K = (kk, q~)
+            for (int pass = 0; pass < npass; ++pass) {
+                uint32_t wrow[MW];
+                int rbase[MW];
+                bool mval[MW];
+#pragma unroll
+                for (int i = 0; i < MW; ++i) {
+                    const int mt = (pass * MW + i) * NWARPS + warp;
+                    mval[i] = mt < nmt;
+                    const int2 ri = rowinfo[min(mt, nmt - 1) * 8 + lr];
+                    wrow[i] = (uint32_t)ri.x; rbase[i] = ri.y * g.rs0;
+                }
+                double acc[MW][NW][2];
+#pragma unroll
+                for (int i = 0; i < MW; ++i)
+#pragma unroll
+                    for (int n = 0; n < NW; ++n) acc[i][n][0] = acc[i][n][1] = 0.0;
+                for (int kk = 0; kk < g.Kket; ++kk) {
+                    const double *Rk = R0 + (long long)kk * g.Kbra * g.rs0;
+                    for (int c = c_first; c < nc1; ++c) {
+                        const double *B = acquire() + lc * NTS + lr;
+                        const int q0 = c * MD_HL_KC1 + lc;
+#pragma unroll 4
+                        for (int k0 = 0; k0 < MD_HL_KC1; k0 += 4) {
+                            const uint32_t wq = s_herm[min(q0 + k0, nhk - 1)];     // rows >= nhk of Hk are zero
+                            double bfr[NW];
+#pragma unroll
+                            for (int n = 0; n < NW; ++n) bfr[n] = B[k0 * NTS + n * 8];
+#pragma unroll
+                            for (int i = 0; i < MW; ++i) {
+                                if (mval[i]) {
+                                    const double a = Rk[rbase[i] + hl_herm_index(wrow[i] + wq)];
+#pragma unroll
+                                    for (int n = 0; n < NW; ++n)
+                                        if (n < nnt) hl_dmma884(acc[i][n][0], acc[i][n][1], a, bfr[n]);
+                                }
+                            }
+                        }
+                        release();
+                    }
+                }
+#pragma unroll
+                for (int i = 0; i < MW; ++i) {
+                    const int mt = (pass * MW + i) * NWARPS + warp;
+                    if (mt < nmt) {
+#pragma unroll
+                        for (int n = 0; n < NW; ++n)
+                            *(double2 *)(Vp + (mt * 8 + lr) * NTS + n * 8 + 2 * lc) = make_double2(acc[i][n][0], acc[i][n][1]);
+                    }
+                }
+            }
+            __syncthreads();
+            // GEMM2 (Eq. 26): rows = ab (MD_HL_MT2 tiles per warp), columns = the cd tile, K = stacked (kb, p~)
+            double c2[MD_HL_MT2][NW][2];
+#pragma unroll
+            for (int t = 0; t < MD_HL_MT2; ++t)
+#pragma unroll
+                for (int n = 0; n < NW; ++n) c2[t][n][0] = c2[t][n][1] = 0.0;
+            for (int c = 0; c < nc2; ++c) {
+                const double *A = acquire() + lc * g.sb + warp * 8 + lr;
+                const double *V = Vp + (c * MD_HL_KC2 + lc) * NTS + lr;
+#pragma unroll
+                for (int ks = 0; ks < MD_HL_KC2 / 4; ++ks) {
+                    double bfr[NW];
+#pragma unroll
+                    for (int n = 0; n < NW; ++n) bfr[n] = V[ks * 4 * NTS + n * 8];
+#pragma unroll
+                    for (int t = 0; t < MD_HL_MT2; ++t) {
+                        if (warp + t * NWARPS < nmt2) {
+                            const double a = A[ks * 4 * g.sb + t * NWARPS * 8];
+#pragma unroll
+                            for (int n = 0; n < NW; ++n)
+                                if (n < nnt) hl_dmma884(c2[t][n][0], c2[t][n][1], a, bfr[n]);
+                        }
+                    }
+                }
+                release();
+            }
+            // S5: the accumulators are the final [ab|cd] tile
+#pragma unroll
+            for (int t = 0; t < MD_HL_MT2; ++t) {
+                const int ab = (warp + t * NWARPS) * 8 + lr;
+                if (ab < g.nab) {
+#pragma unroll
+                    for (int n = 0; n < NW; ++n) {
+                        const int cd = cd0 + n * 8 + 2 * lc;
+                        double *o = out + ab * g.s_ab + cd * g.s_cd;
+                        if (cd < g.ncd) o[0] = c2[t][n][0];
+                        if (cd + 1 < g.ncd) o[g.s_cd] = c2[t][n][1];
+                    }
+                }
+            }
+            __syncthreads();                               // [p~|cd] is rewritten by the next tile
+        }
+    }
+}
+
+}  // namespace mdb

@@ -1,0 +1,131 @@
+// hl_inst.cu -- host side of the high-l quartet kernel: tile selection, shared-memory carve-up, launch.
+#include <algorithm>
+#include <cstdio>
+#include <cstdlib>
+
+#include "hl_api.cuh"
+#include "hl_reg.cuh"
+
+namespace mdb {
+
+namespace {
+HlFn g_hl[2][5][5];                   // [0]: 4 warps, [1]: 8 warps; [MW][NW]
+int g_hl_max_smem = 227 * 1024;
+}  // namespace
+HlFn *hl_table() { return &g_hl[0][0][0]; }
+
+cudaError_t hl_init(int max_smem, const uint32_t *herm, const double *solid) {
+    g_hl_max_smem = max_smem;
+    cudaError_t e;
+    if ((e = hl_register_w4(max_smem, herm, solid)) != cudaSuccess) return e;
+    return hl_register_w8(max_smem, herm, solid);
+}
+
+namespace {
+
+struct HlPlan {
+    HlArgs a;
+    int MW, NW, warps, ctas, npass;
+    size_t smem, scratch_bytes;
+    unsigned grid;
+};
+
+inline int even_up(int x) { return x + (x & 1); }
+inline int up16(int x) { return (x + 15) / 16 * 16; }
+
+bool make_plan(const HlCall &c, int nsm, HlPlan &P) {
+    HlArgs &a = P.a;
+    a.bra = c.bra; a.ket = c.ket; a.pure = c.pure;
+    a.la = c.bra.a.l; a.lb = c.bra.single ? 0 : c.bra.b.l; a.lc = c.ket.a.l; a.ld = c.ket.single ? 0 : c.ket.b.l;
+    a.Ka = c.bra.a.K; a.Kb = c.bra.single ? 1 : c.bra.b.K; a.Kc = c.ket.a.K; a.Kd = c.ket.single ? 1 : c.ket.b.K;
+    a.Kbra = a.Ka * a.Kb; a.Kket = a.Kc * a.Kd;
+    a.Lb = a.la + a.lb; a.Lk = a.lc + a.ld;
+    a.nab = ncomp(a.la, c.pure) * ncomp(a.lb, c.pure); a.ncd = ncomp(a.lc, c.pure) * ncomp(a.ld, c.pure);
+    a.nhb = nherm(a.Lb); a.nhk = nherm(a.Lk);
+    a.mrows = a.Kbra * a.nhb; a.mrows_pad = (a.mrows + 7) / 8 * 8;
+    a.nhk_pad = (a.nhk + MD_HL_KC1 - 1) / MD_HL_KC1 * MD_HL_KC1;
+    const int nmt2 = (a.nab + 7) / 8, nmt = a.mrows_pad / 8;
+    a.sb = (8 * nmt2 - 4 + 15) / 16 * 16 + 4;
+    a.q_first = (c.ket.single && c.pure) ? nherm(a.lc - 1) / MD_HL_KC1 * MD_HL_KC1 : 0;
+    a.qidx = c.qidx; a.nq = c.nq; a.nket = c.ket.npairs; a.out = c.out;
+    a.s_q = c.s_q; a.s_bi = c.s_bi; a.s_ki = c.s_ki; a.s_ab = c.s_ab; a.s_cd = c.s_cd;
+    a.boys_tab = c.boys_tab; a.rlut = c.rlut;
+    const int L = a.Lb + a.Lk, nR = a.Kbra * a.Kket;
+    a.rs0 = even_up(nherm(L)); a.rs1 = even_up(L > 0 ? nherm(L - 1) : 1);
+
+    // cd tile width: as few tiles as possible, at most 4 column tiles of 8 per warp
+    const int nnt_total = (a.ncd + 7) / 8;
+    const int ntile = (nnt_total + 3) / 4;
+    int NW = (nnt_total + ntile - 1) / ntile;
+    int warps, MW;
+    if (nmt <= 12 && nmt2 <= 4 * MD_HL_MT2) { warps = 4; MW = std::min(3, (nmt + 3) / 4); }
+    else { warps = 8; MW = std::min(4, (nmt + 7) / 8); }
+    if (const char *f = getenv("MD_HL_FORCE")) {           // measurement override: "MW,NW,warps"
+        int m, n, w;
+        if (sscanf(f, "%d,%d,%d", &m, &n, &w) == 3 && (w == 4 || w == 8) && m >= 1 && m <= (w == 4 ? 3 : 4) && n >= 1 && n <= 4) {
+            MW = m; NW = n; warps = w;
+        }
+    }
+    if (nmt2 > warps * MD_HL_MT2) return false;            // the [ab|cd] tile must fit the GEMM2 accumulators
+    const int NT = 8 * NW, NTS = NT + 4;
+    a.ntile = (a.ncd + NT - 1) / NT;
+    P.MW = MW; P.NW = NW; P.warps = warps;
+    P.npass = (nmt + warps * MW - 1) / (warps * MW);
+
+    a.ring_stage = up16(std::max(MD_HL_KC1 * NTS, MD_HL_KC2 * a.sb));
+    const int esz_b = (a.la + 1) * (a.lb + 1) * (a.Lb + 1), esz_k = (a.lc + 1) * (a.ld + 1) * (a.Lk + 1);
+    const int t1_b = c.pure ? ncart(a.la) * nsolid(a.lb) : 0, t1_k = c.pure ? ncart(a.lc) * nsolid(a.ld) : 0;
+    const int s1_need = std::max(3 * esz_b + 8 * t1_b, 3 * esz_k + 8 * t1_k);
+    int ov = std::max(a.mrows_pad * NTS, nR * a.rs1);
+    ov = std::max(ov, s1_need - MD_HL_STAGES * a.ring_stage);
+    a.ov_doubles = up16(ov);
+    int o = 0;
+    a.o_herm = o; o += even_up(nherm(std::max(a.Lb, a.Lk))) / 2 + 1;
+    a.o_rowinfo = o; o += a.mrows_pad;
+    a.o_ct = o; o += 4 * 28 * MD_HL_CSTR;
+    a.o_hdr = o; o += 4 * (a.Kbra + a.Kket);
+    a.o_bar = o; o += 2 * MD_HL_STAGES;
+    a.o_r0 = o; o += nR * a.rs0;
+    a.o_g0 = o; o += even_up(nR * (L + 1));
+    a.o_pq = o; o += even_up(nR * 3);
+    o = up16(o);
+    a.o_ov = o; o += a.ov_doubles;
+    a.o_ring = o; o += MD_HL_STAGES * a.ring_stage;
+    a.total = o;
+    P.smem = (size_t)o * 8;
+    if (P.smem > (size_t)g_hl_max_smem) return false;
+    if (!hl_table()[((warps == 8) * 5 + MW) * 5 + NW]) return false;
+
+    const long long hb_doubles = (long long)a.mrows_pad * a.sb;
+    const long long hk_doubles = (long long)a.ntile * a.Kket * a.nhk_pad * NTS;
+    a.off_hk = (hb_doubles + 15) / 16 * 16;
+    a.scratch_stride = (a.off_hk + hk_doubles + 15) / 16 * 16;
+    const int by_regs = warps == 4 ? 3 : (MW <= 2 ? 2 : 1);
+    P.ctas = (int)std::max<size_t>(1, std::min<size_t>(by_regs, (size_t)(g_hl_max_smem + 1024) / (P.smem + 1024)));
+    P.grid = (unsigned)std::min<long long>(c.nq, (long long)nsm * P.ctas);
+    P.scratch_bytes = (size_t)P.grid * a.scratch_stride * 8;
+    return true;
+}
+
+}  // namespace
+
+int hl_plan(const HlCall &c, int nsm, size_t *scratch_bytes) {
+    HlPlan P;
+    if (!make_plan(c, nsm, P)) return 0;
+    *scratch_bytes = P.scratch_bytes;
+    return 1;
+}
+
+cudaError_t hl_launch(const HlCall &c, int nsm, void *scratch, cudaStream_t st, int *info) {
+    HlPlan P;
+    if (!make_plan(c, nsm, P)) return cudaErrorInvalidConfiguration;
+    P.a.scratch = (double *)scratch;
+    hl_table()[((P.warps == 8) * 5 + P.MW) * 5 + P.NW]<<<P.grid, 32 * P.warps, P.smem, st>>>(P.a);
+    if (info) {
+        info[0] = P.MW; info[1] = P.NW; info[2] = P.warps; info[3] = (int)P.smem; info[4] = P.ctas; info[5] = P.npass;
+        info[6] = P.a.ntile; info[7] = (int)P.grid;
+    }
+    return cudaGetLastError();
+}
+
+}  // namespace mdb

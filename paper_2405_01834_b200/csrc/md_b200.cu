@@ -14,6 +14,7 @@
 #include "common.cuh"
 #include "fused_api.cuh"
 #include "generic.cuh"
+#include "hl_api.cuh"
 #include "mma_api.cuh"
 #include "pair.cuh"
 #include "warp.cuh"
@@ -34,6 +35,7 @@ struct State {
     int last_launches = 0;
     int last_mma_info[8] = {0};
     int last_f2_info[8] = {0};
+    int last_hl_info[8] = {0};
     int nsm = 148;
     int max_smem = 227 * 1024;
     char cuda_err[256] = "";
@@ -308,6 +310,24 @@ int run(const PairView &b, const PairView &k, long long nq, const int32_t *qidx,
         }
         if (r < 0) return r;
     }
+    if (S.variant == MD_VARIANT_AUTO || S.variant == MD_VARIANT_HL) {
+        // Classes with an l >= 3 shell: the one-launch high-l kernel (hl.cuh) when its tiles fit the (class, K).
+        HlCall c;
+        c.bra = b; c.ket = k; c.pure = pure; c.qidx = qidx; c.nq = nq; c.out = out;
+        out_strides(layout, qidx != nullptr, b.npairs, k.npairs, s.nab, s.ncd, c.s_q, c.s_bi, c.s_ki, c.s_ab, c.s_cd);
+        c.boys_tab = S.boys_tab; c.rlut = fused_rlut();
+        size_t need = 0;
+        const bool small = s.la + s.lb + s.lc + s.ld <= MD_WARP_LMAX && s.nhb * s.ncd <= MD_WARP_HALF;   // the warp kernel's classes
+        if ((S.variant == MD_VARIANT_HL || !small) && hl_plan(c, S.nsm, &need)) {
+            void *ws = nullptr;
+            int e = sc.get(need, &ws);
+            if (e) return e;
+            CK(hl_launch(c, S.nsm, ws, st, S.last_hl_info));
+            S.last_launches++;
+            S.last_variant = MD_VARIANT_HL;
+            return MD_OK;
+        }
+    }
     return run_generic(b, k, nq, qidx, pure, layout, out, st, S.variant != MD_VARIANT_GENERIC, sc);
 }
 
@@ -371,6 +391,7 @@ int md_init(void) {
     CK(fused_init(S.max_smem));
     CK(fused2_init(S.max_smem));
     CK(mma_init(S.max_smem));
+    CK(hl_init(S.max_smem, herm.data(), solid.data()));
     CK(cudaDeviceSynchronize());
     S.init = true;
     S.device = dev;
@@ -420,7 +441,7 @@ int md_set_workspace(void *p, size_t bytes) {
     return MD_OK;
 }
 int md_set_variant(int v) {
-    if (v < MD_VARIANT_AUTO || v > MD_VARIANT_WARP) return MD_EINVAL;
+    if (v < MD_VARIANT_AUTO || v > MD_VARIANT_HL) return MD_EINVAL;
     S.variant = v;
     return MD_OK;
 }
