@@ -16,16 +16,17 @@
 //   S5  the accumulators of GEMM2 are the final [ab|cd] tile: stored once, no read-modify-write.
 // tcgen05 has no FP64 kind, so mma.sync is the only tensor path FP64 has on sm_100a.
 #pragma once
+#include <type_traits>
+
 #include "boys.cuh"
 #include "common.cuh"
 
 namespace mdb {
 
 #define MD_HL_KC1 32          // ket Hermite rows per ring chunk of GEMM1
-#define MD_HL_KC2 8           // stacked bra rows per ring chunk of GEMM2
 #define MD_HL_STAGES 4
 #define MD_HL_MT2 3           // ab row tiles per warp in GEMM2 (register-resident output)
-#define MD_HL_CSTR 14         // row stride of the transposed Cartesian->solid tables [cart][m], 13 padded to 14
+#define MD_HL_CSTR 16         // row stride of the transposed Cartesian->solid tables [cart][m], zero-padded
 
 struct HlArgs {
     PairView bra, ket;
@@ -33,7 +34,8 @@ struct HlArgs {
     int la, lb, lc, ld;                  // ld = 0 for a one-centre ket
     int Ka, Kb, Kc, Kd, Kbra, Kket;
     int Lb, Lk, nab, ncd, nhb, nhk;
-    int mrows, mrows_pad;                // stacked rows (kb, p~) of [p~|cd]; padded to a multiple of 8
+    int mrows, mrows_pad;                // stacked rows (kb, p~) of [p~|cd]; padded to a multiple of kc2
+    int kc2;                             // stacked bra rows per ring chunk of GEMM2: 8 or 16
     int nhk_pad;                         // ket Hermite rows padded to MD_HL_KC1
     int sb;                              // row stride of Hb in the scratch: >= 8*ceil(nab/8), = 4 mod 16
     int ntile;                           // cd tiles
@@ -162,56 +164,125 @@ __device__ __forceinline__ void hl_build_H(int la, int lb, int pure, bool neg, d
         __syncthreads();
         return;
     }
+    // Both stages on the FP64 tensor path (mma.sync.m8n8k4.f64), 8 x 8 tiles, K steps of 4:
+    //   stage A  rows (p~, a), columns mb, K = b: a lane forms its own A element E^{ab}_{p~} from the three axis tables;
+    //            the B fragments C^{lb}[b][mb] are class constants held in registers.  A K step whose 32 elements all
+    //            vanish (Eq. 14) is skipped.
+    //   stage B  per p~: rows ma, columns mb, K = a: A fragments C^{la}[a][ma] in registers, B fragments from T1.
     const int nsa = nsolid(la), nsb = nsolid(lb);
-    const int pchunk = max(1, min(nh, t1cap / (nca * nsb)));
+    const int lane = tid & 31, warp = tid >> 5, lr = lane >> 2, lc = lane & 3;
+    constexpr int NWARPS = NTHR / 32, TS = 20;              // T1 row stride: 16 columns + 4 (conflict-free fragments)
+    const int ntb = (nsb + 7) >> 3, nta = (nsa + 7) >> 3;   // column tiles of mb, row tiles of ma (1 or 2)
+    const int ksb = (ncb + 3) >> 2, ksa = (nca + 3) >> 2;   // K steps over b and over a (<= 7)
+    const int pchunk = max(1, min(nh, t1cap / (nca * TS)));
+    double cbf[7][2], caf[7][2];                            // constant fragments: C^{lb}[b][mb], C^{la}[a][ma]
+    uint32_t boff[7];                                       // per K step: offsets bx*nt | by*nt << 8 | bz*nt << 16 of b = 4k + lc
+#pragma unroll
+    for (int k = 0; k < 7; ++k) {
+        const int b = 4 * k + lc;
+        int bx = 0, by = 0, bz = 0;
+        if (b < ncb) unpack_tuv(cb[b], bx, by, bz);
+        boff[k] = (uint32_t)(bx * nt) | (uint32_t)(by * nt) << 8 | (uint32_t)(bz * nt) << 16;
+#pragma unroll
+        for (int n = 0; n < 2; ++n) {
+            cbf[k][n] = b < ncb ? CbT[b * MD_HL_CSTR + 8 * n + lr] : 0.0;
+            caf[k][n] = b < nca ? CaT[b * MD_HL_CSTR + 8 * n + lr] : 0.0;    // same lane pattern: a = 4k + lc, ma = 8n + lr
+        }
+    }
     for (int h0 = 0; h0 < nh; h0 += pchunk) {
         const int hc = min(pchunk, nh - h0);
-        for (int e = tid; e < hc * nca; e += NTHR) {
-            const int ih = e / nca, a = e - ih * nca;
+        const int nrows = hc * nca, nmt = (nrows + 7) >> 3;
+        for (int mt = warp; mt < nmt; mt += NWARPS) {
+            const int r = mt * 8 + lr;
+            const bool rv = r < nrows;
+            const int rr = rv ? r : nrows - 1;
+            const int ih = rr / nca, a = rr - ih * nca;
             int t, u, v, ax, ay, az;
             unpack_tuv(s_herm[h0 + ih], t, u, v);
             unpack_tuv(ca[a], ax, ay, az);
             const double *ex = Ex + ax * (lb + 1) * nt + t, *ey = Ey + ay * (lb + 1) * nt + u, *ez = Ez + az * (lb + 1) * nt + v;
-            double acc[13];
+            double c[2][2] = {{0.0, 0.0}, {0.0, 0.0}};
+            // all operands first (21 loads in flight), then the votes, then the tensor-core steps
+            double x[7];
+            uint32_t live = 0;
 #pragma unroll
-            for (int m = 0; m < 13; ++m) acc[m] = 0.0;
-            for (int b = 0; b < ncb; ++b) {
-                int bx, by, bz;
-                unpack_tuv(cb[b], bx, by, bz);
-                const double x = ex[bx * nt] * ey[by * nt] * ez[bz * nt];
-                if (!__any_sync(__activemask(), x != 0.0)) continue;
-                const double *c = CbT + b * MD_HL_CSTR;
-#pragma unroll
-                for (int m = 0; m < 13; ++m)
-                    if (m < nsb) acc[m] = fma(c[m], x, acc[m]);
+            for (int k = 0; k < 7; ++k) {
+                const uint32_t o = boff[k];
+                x[k] = ex[o & 0xff] * ey[o >> 8 & 0xff] * ez[o >> 16];
+                if (!rv || 4 * k + lc >= ncb) x[k] = 0.0;
             }
-            double *o = T1 + (size_t)e * nsb;
 #pragma unroll
-            for (int m = 0; m < 13; ++m)
-                if (m < nsb) o[m] = acc[m];
+            for (int k = 0; k < 7; ++k) live |= (__any_sync(0xffffffffu, x[k] != 0.0) ? 1u : 0u) << k;
+#pragma unroll
+            for (int k = 0; k < 7; ++k) {
+                if (live >> k & 1) {
+                    hl_dmma884(c[0][0], c[0][1], x[k], cbf[k][0]);
+                    if (ntb > 1) hl_dmma884(c[1][0], c[1][1], x[k], cbf[k][1]);
+                }
+            }
+            double *o = T1 + (size_t)r * TS + 2 * lc;
+            if (rv) {
+                *(double2 *)o = make_double2(c[0][0], c[0][1]);
+                if (ntb > 1) *(double2 *)(o + 8) = make_double2(c[1][0], c[1][1]);
+            }
         }
         __syncthreads();
-        for (int e = tid; e < hc * nsb; e += NTHR) {
-            const int ih = e / nsb, mb = e - ih * nsb;
-            const double *t1 = T1 + (size_t)ih * nca * nsb + mb;
-            double acc[13];
+        for (int ih = warp; ih < hc; ih += NWARPS) {
+            const double *t1 = T1 + (size_t)ih * nca * TS + lr;
+            double c[2][2][2] = {{{0.0, 0.0}, {0.0, 0.0}}, {{0.0, 0.0}, {0.0, 0.0}}};      // [ma tile][mb tile][2]
+            double b0[7], b1[7];
+            uint32_t live = 0;
 #pragma unroll
-            for (int m = 0; m < 13; ++m) acc[m] = 0.0;
-            for (int a = 0; a < nca; ++a) {
-                const double y = t1[a * nsb];
-                if (!__any_sync(__activemask(), y != 0.0)) continue;
-                const double *c = CaT + a * MD_HL_CSTR;
-#pragma unroll
-                for (int m = 0; m < 13; ++m)
-                    if (m < nsa) acc[m] = fma(c[m], y, acc[m]);
+            for (int k = 0; k < 7; ++k) {
+                const int a = min(4 * k + lc, nca - 1);
+                b0[k] = t1[a * TS];
+                b1[k] = t1[a * TS + 8];
+                if (4 * k + lc >= nca) { b0[k] = 0.0; b1[k] = 0.0; }
+                if (ntb == 1) b1[k] = 0.0;
             }
-            const double s = (neg && (s_herm[h0 + ih] >> 24 & 1)) ? -coef : coef;
 #pragma unroll
-            for (int m = 0; m < 13; ++m)
-                if (m < nsa) *dst(h0 + ih, m * nsb + mb) = s * acc[m];
+            for (int k = 0; k < 7; ++k) live |= (__any_sync(0xffffffffu, b0[k] != 0.0 || b1[k] != 0.0) ? 1u : 0u) << k;
+#pragma unroll
+            for (int k = 0; k < 7; ++k) {
+                if (live >> k & 1) {
+                    hl_dmma884(c[0][0][0], c[0][0][1], caf[k][0], b0[k]);
+                    if (ntb > 1) hl_dmma884(c[0][1][0], c[0][1][1], caf[k][0], b1[k]);
+                    if (nta > 1) {
+                        hl_dmma884(c[1][0][0], c[1][0][1], caf[k][1], b0[k]);
+                        if (ntb > 1) hl_dmma884(c[1][1][0], c[1][1][1], caf[k][1], b1[k]);
+                    }
+                }
+            }
+            const double sgn = (neg && (s_herm[h0 + ih] >> 24 & 1)) ? -coef : coef;
+#pragma unroll
+            for (int i = 0; i < 2; ++i)
+#pragma unroll
+                for (int n = 0; n < 2; ++n) {
+                    const int ma = 8 * i + lr, mb = 8 * n + 2 * lc;
+                    if (ma < nsa && mb < nsb) *dst(h0 + ih, ma * nsb + mb) = sgn * c[i][n][0];
+                    if (ma < nsa && mb + 1 < nsb) *dst(h0 + ih, ma * nsb + mb + 1) = sgn * c[i][n][1];
+                }
         }
         __syncthreads();
     }
+}
+
+// One K step (4 ket Hermite rows) of GEMM1 for a warp's MW x NW tiles: the A elements [p~+q~]^(0) are gathered from
+// the tensor, the B fragments come from the ring.  FULLN: all NW column tiles of the cd tile exist (no guards, so the
+// compiler can overlap the index arithmetic of one step with the tensor-core instructions of the previous one).
+template <int MW, int NW, bool FULLN>
+__device__ __forceinline__ void hl_gemm1_step(double (&acc)[MW][NW][2], const double *B, const double *Rk,
+                                              const int (&rbase)[MW], const uint32_t (&wrow)[MW], uint32_t wq, int nnt) {
+    double bfr[NW], a[MW];
+#pragma unroll
+    for (int n = 0; n < NW; ++n) bfr[n] = B[n * 8];
+#pragma unroll
+    for (int i = 0; i < MW; ++i) a[i] = Rk[rbase[i] + hl_herm_index(wrow[i] + wq)];
+#pragma unroll
+    for (int i = 0; i < MW; ++i)
+#pragma unroll
+        for (int n = 0; n < NW; ++n)
+            if (FULLN || n < nnt) hl_dmma884(acc[i][n][0], acc[i][n][1], a[i], bfr[n]);
 }
 
 // Order in which one quartet's H chunks pass through the ring: for every cd tile, for every row pass of GEMM1 the
@@ -222,7 +293,7 @@ struct HlStream {
 };
 
 template <int MW, int NW, int NWARPS>
-__global__ void __launch_bounds__(32 * NWARPS, (NWARPS == 4 ? 3 : (MW <= 2 ? 2 : 1))) hl_kernel(HlArgs g) {
+__global__ void __launch_bounds__(32 * NWARPS, (NWARPS == 4 ? 3 : 1)) hl_kernel(HlArgs g) {
     constexpr int NTHR = 32 * NWARPS, NT = 8 * NW, NTS = NT + 4, ST = MD_HL_STAGES;
     extern __shared__ double sm[];
     uint32_t *s_herm = (uint32_t *)(sm + g.o_herm);
@@ -242,16 +313,18 @@ __global__ void __launch_bounds__(32 * NWARPS, (NWARPS == 4 ? 3 : (MW <= 2 ? 2 :
     double *scr = g.scratch + (long long)blockIdx.x * g.scratch_stride;
     double *hb = scr, *hk = scr + g.off_hk;
     const int nmt = g.mrows_pad >> 3, npass = (nmt + NWARPS * MW - 1) / (NWARPS * MW);
-    const int nc1 = g.nhk_pad / MD_HL_KC1, c_first = g.q_first / MD_HL_KC1, nc2 = g.mrows_pad / MD_HL_KC2;
+    const int nc1 = g.nhk_pad / MD_HL_KC1, c_first = g.q_first / MD_HL_KC1, nc2 = g.mrows_pad / g.kc2;
     const int nmt2 = (g.nab + 7) >> 3;
     const long long hk_tile = (long long)g.Kket * g.nhk_pad * NTS;
-    const uint32_t bytes1 = MD_HL_KC1 * NTS * 8, bytes2 = MD_HL_KC2 * g.sb * 8;
+    const uint32_t bytes1 = MD_HL_KC1 * NTS * 8, bytes2 = g.kc2 * g.sb * 8;
 
     // ---- once per CTA: constant tables, barriers, zeroed scratch (its padding is never written again) ----
     {
         const int nhm = nherm(max(g.Lb, g.Lk));
         for (int i = tid; i < nhm; i += NTHR) s_herm[i] = c_herm[i];
         const int ls[4] = {g.la, g.lb, g.lc, g.ld};
+        for (int i = tid; i < 4 * CTS; i += NTHR) CT[i] = 0.0;
+        __syncthreads();
         for (int s = 0; s < 4; ++s) {
             const int l = ls[s], nc = ncart(l), ns = nsolid(l);
             for (int i = tid; i < nc * ns; i += NTHR) {
@@ -284,7 +357,7 @@ __global__ void __launch_bounds__(32 * NWARPS, (NWARPS == 4 ? 3 : (MW <= 2 ? 2 :
             bytes = bytes1;
             if (++ps.c == nc1) { ps.c = c_first; if (++ps.kk == g.Kket) { ps.kk = 0; if (++ps.pass == npass) { ps.pass = 0; ps.c2 = 0; } } }
         } else {
-            src = hb + (long long)ps.c2 * MD_HL_KC2 * g.sb;
+            src = hb + (long long)ps.c2 * g.kc2 * g.sb;
             bytes = bytes2;
             if (++ps.c2 == nc2) { ps.c2 = -1; ++ps.j; }
         }
@@ -320,8 +393,8 @@ __global__ void __launch_bounds__(32 * NWARPS, (NWARPS == 4 ? 3 : (MW <= 2 ? 2 :
             long long i1 = ip, i2 = ip;
             if (pv.idx) { i1 = pv.idx[2 * ip]; i2 = pv.idx[2 * ip + 1]; }
             const int esz = (l1 + 1) * (l2 + 1) * (l1 + l2 + 1);
-            double *E = ov, *T1 = ov + 3 * esz;
-            const int t1cap = g.ov_doubles + ST * g.ring_stage - 3 * esz;
+            double *E = ov, *T1 = ov + ((3 * esz + 1) & ~1);           // 16-byte aligned rows for the fragment stores
+            const int t1cap = g.ov_doubles + ST * g.ring_stage - ((3 * esz + 1) & ~1);
             for (int kp = 0; kp < K1 * K2; ++kp) {
                 const int k1 = kp / K2, k2 = kp - k1 * K2;
                 const double za = pv.a.exps[i1 * K1 + k1];
@@ -389,21 +462,19 @@ __global__ void __launch_bounds__(32 * NWARPS, (NWARPS == 4 ? 3 : (MW <= 2 ? 2 :
             __syncthreads();
             for (int m = L - 1; m >= 0; --m) {
                 const int ne = nherm(L - m);
-                for (int s = warp; s < nR; s += NWARPS) {
+                for (int it = tid; it < nR * ne; it += NTHR) {
+                    const int s = it / ne, e = it - s * ne;
                     const double *old = (m & 1) ? R0 + s * g.rs0 : R1 + s * g.rs1;
                     double *nw = (m & 1) ? R1 + s * g.rs1 : R0 + s * g.rs0;
-                    const double *pq = PQ + 3 * s;
-                    for (int e = lane; e < ne; e += 32) {
-                        const uint32_t w = __ldg(&lut[e].x);
-                        double val;
-                        if (e == 0) val = G0[s * (L + 1) + m];
-                        else {
-                            val = pq[w >> 24 & 3] * old[w & 0xfff];
-                            const int cf = w >> 26;
-                            if (cf) val = fma((double)cf, old[w >> 12 & 0xfff], val);
-                        }
-                        nw[e] = val;
+                    const uint32_t w = __ldg(&lut[e].x);
+                    double val;
+                    if (e == 0) val = G0[s * (L + 1) + m];
+                    else {
+                        val = PQ[3 * s + (w >> 24 & 3)] * old[w & 0xfff];
+                        const int cf = w >> 26;
+                        if (cf) val = fma((double)cf, old[w >> 12 & 0xfff], val);
                     }
+                    nw[e] = val;
                 }
                 __syncthreads();
             }
@@ -417,11 +488,9 @@ __global__ void __launch_bounds__(32 * NWARPS, (NWARPS == 4 ? 3 : (MW <= 2 ? 2 :
             for (int pass = 0; pass < npass; ++pass) {
                 uint32_t wrow[MW];
                 int rbase[MW];
-                bool mval[MW];
 #pragma unroll
-                for (int i = 0; i < MW; ++i) {
+                for (int i = 0; i < MW; ++i) {                 // row tiles past the end compute on a clamped row; not stored
                     const int mt = (pass * MW + i) * NWARPS + warp;
-                    mval[i] = mt < nmt;
                     const int2 ri = rowinfo[min(mt, nmt - 1) * 8 + lr];
                     wrow[i] = (uint32_t)ri.x; rbase[i] = ri.y * g.rs0;
                 }
@@ -435,21 +504,23 @@ __global__ void __launch_bounds__(32 * NWARPS, (NWARPS == 4 ? 3 : (MW <= 2 ? 2 :
                     for (int c = c_first; c < nc1; ++c) {
                         const double *B = acquire() + lc * NTS + lr;
                         const int q0 = c * MD_HL_KC1 + lc;
-#pragma unroll 4
-                        for (int k0 = 0; k0 < MD_HL_KC1; k0 += 4) {
-                            const uint32_t wq = s_herm[min(q0 + k0, nhk - 1)];     // rows >= nhk of Hk are zero
-                            double bfr[NW];
+                        const int nsteps = min(MD_HL_KC1 / 4, (nhk - c * MD_HL_KC1 + 3) >> 2);   // rows >= nhk of Hk are zero
+                        if (nsteps == MD_HL_KC1 / 4) {
+                            uint32_t wq[MD_HL_KC1 / 4];
 #pragma unroll
-                            for (int n = 0; n < NW; ++n) bfr[n] = B[k0 * NTS + n * 8];
+                            for (int k = 0; k < MD_HL_KC1 / 4; ++k) wq[k] = s_herm[min(q0 + 4 * k, nhk - 1)];
+                            if (nnt == NW) {
 #pragma unroll
-                            for (int i = 0; i < MW; ++i) {
-                                if (mval[i]) {
-                                    const double a = Rk[rbase[i] + hl_herm_index(wrow[i] + wq)];
+                                for (int k = 0; k < MD_HL_KC1 / 4; ++k)
+                                    hl_gemm1_step<MW, NW, true>(acc, B + 4 * k * NTS, Rk, rbase, wrow, wq[k], nnt);
+                            } else {
 #pragma unroll
-                                    for (int n = 0; n < NW; ++n)
-                                        if (n < nnt) hl_dmma884(acc[i][n][0], acc[i][n][1], a, bfr[n]);
-                                }
+                                for (int k = 0; k < MD_HL_KC1 / 4; ++k)
+                                    hl_gemm1_step<MW, NW, false>(acc, B + 4 * k * NTS, Rk, rbase, wrow, wq[k], nnt);
                             }
+                        } else {
+                            for (int k = 0; k < nsteps; ++k)
+                                hl_gemm1_step<MW, NW, false>(acc, B + 4 * k * NTS, Rk, rbase, wrow, s_herm[min(q0 + 4 * k, nhk - 1)], nnt);
                         }
                         release();
                     }
@@ -471,25 +542,46 @@ __global__ void __launch_bounds__(32 * NWARPS, (NWARPS == 4 ? 3 : (MW <= 2 ? 2 :
             for (int t = 0; t < MD_HL_MT2; ++t)
 #pragma unroll
                 for (int n = 0; n < NW; ++n) c2[t][n][0] = c2[t][n][1] = 0.0;
-            for (int c = 0; c < nc2; ++c) {
-                const double *A = acquire() + lc * g.sb + warp * 8 + lr;
-                const double *V = Vp + (c * MD_HL_KC2 + lc) * NTS + lr;
+            // specialised on the number of ab row tiles this warp owns (TC) and on a full cd tile: no guards inside
+            auto gemm2 = [&](auto tc, auto full) {
+                constexpr int TC = decltype(tc)::value;
+                constexpr bool FULLN = decltype(full)::value;
+                for (int c = 0; c < nc2; ++c) {
+                    const double *A = acquire() + lc * g.sb + warp * 8 + lr;
+                    const double *V = Vp + (c * g.kc2 + lc) * NTS + lr;
+                    for (int u = 0; u < g.kc2; u += 8) {
 #pragma unroll
-                for (int ks = 0; ks < MD_HL_KC2 / 4; ++ks) {
-                    double bfr[NW];
+                        for (int ks = 0; ks < 2; ++ks) {
+                            double bfr[NW], a[TC > 0 ? TC : 1];
 #pragma unroll
-                    for (int n = 0; n < NW; ++n) bfr[n] = V[ks * 4 * NTS + n * 8];
+                            for (int n = 0; n < NW; ++n) bfr[n] = V[(u + ks * 4) * NTS + n * 8];
 #pragma unroll
-                    for (int t = 0; t < MD_HL_MT2; ++t) {
-                        if (warp + t * NWARPS < nmt2) {
-                            const double a = A[ks * 4 * g.sb + t * NWARPS * 8];
+                            for (int t = 0; t < TC; ++t) a[t] = A[(u + ks * 4) * g.sb + t * NWARPS * 8];
 #pragma unroll
-                            for (int n = 0; n < NW; ++n)
-                                if (n < nnt) hl_dmma884(c2[t][n][0], c2[t][n][1], a, bfr[n]);
+                            for (int t = 0; t < TC; ++t)
+#pragma unroll
+                                for (int n = 0; n < NW; ++n)
+                                    if (FULLN || n < nnt) hl_dmma884(c2[t][n][0], c2[t][n][1], a[t], bfr[n]);
                         }
                     }
+                    release();
                 }
-                release();
+            };
+            {
+                const int tc = max(0, (nmt2 - warp + NWARPS - 1) / NWARPS);
+                using std::integral_constant;
+                using T = std::true_type; using F = std::false_type;
+                if (nnt == NW) {
+                    if (tc >= 3) gemm2(integral_constant<int, 3>{}, T{});
+                    else if (tc == 2) gemm2(integral_constant<int, 2>{}, T{});
+                    else if (tc == 1) gemm2(integral_constant<int, 1>{}, T{});
+                    else gemm2(integral_constant<int, 0>{}, T{});
+                } else {
+                    if (tc >= 3) gemm2(integral_constant<int, 3>{}, F{});
+                    else if (tc == 2) gemm2(integral_constant<int, 2>{}, F{});
+                    else if (tc == 1) gemm2(integral_constant<int, 1>{}, F{});
+                    else gemm2(integral_constant<int, 0>{}, F{});
+                }
             }
             // S5: the accumulators are the final [ab|cd] tile
 #pragma unroll

@@ -42,9 +42,9 @@ bool make_plan(const HlCall &c, int nsm, HlPlan &P) {
     a.Lb = a.la + a.lb; a.Lk = a.lc + a.ld;
     a.nab = ncomp(a.la, c.pure) * ncomp(a.lb, c.pure); a.ncd = ncomp(a.lc, c.pure) * ncomp(a.ld, c.pure);
     a.nhb = nherm(a.Lb); a.nhk = nherm(a.Lk);
-    a.mrows = a.Kbra * a.nhb; a.mrows_pad = (a.mrows + 7) / 8 * 8;
+    a.mrows = a.Kbra * a.nhb;
     a.nhk_pad = (a.nhk + MD_HL_KC1 - 1) / MD_HL_KC1 * MD_HL_KC1;
-    const int nmt2 = (a.nab + 7) / 8, nmt = a.mrows_pad / 8;
+    const int nmt2 = (a.nab + 7) / 8, nmt = (a.mrows + 7) / 8;
     a.sb = (8 * nmt2 - 4 + 15) / 16 * 16 + 4;
     a.q_first = (c.ket.single && c.pure) ? nherm(a.lc - 1) / MD_HL_KC1 * MD_HL_KC1 : 0;
     a.qidx = c.qidx; a.nq = c.nq; a.nket = c.ket.npairs; a.out = c.out;
@@ -70,37 +70,44 @@ bool make_plan(const HlCall &c, int nsm, HlPlan &P) {
     const int NT = 8 * NW, NTS = NT + 4;
     a.ntile = (a.ncd + NT - 1) / NT;
     P.MW = MW; P.NW = NW; P.warps = warps;
-    P.npass = (nmt + warps * MW - 1) / (warps * MW);
 
-    a.ring_stage = up16(std::max(MD_HL_KC1 * NTS, MD_HL_KC2 * a.sb));
     const int esz_b = (a.la + 1) * (a.lb + 1) * (a.Lb + 1), esz_k = (a.lc + 1) * (a.ld + 1) * (a.Lk + 1);
-    const int t1_b = c.pure ? ncart(a.la) * nsolid(a.lb) : 0, t1_k = c.pure ? ncart(a.lc) * nsolid(a.ld) : 0;
-    const int s1_need = std::max(3 * esz_b + 8 * t1_b, 3 * esz_k + 8 * t1_k);
-    int ov = std::max(a.mrows_pad * NTS, nR * a.rs1);
-    ov = std::max(ov, s1_need - MD_HL_STAGES * a.ring_stage);
-    a.ov_doubles = up16(ov);
-    int o = 0;
-    a.o_herm = o; o += even_up(nherm(std::max(a.Lb, a.Lk))) / 2 + 1;
-    a.o_rowinfo = o; o += a.mrows_pad;
-    a.o_ct = o; o += 4 * 28 * MD_HL_CSTR;
-    a.o_hdr = o; o += 4 * (a.Kbra + a.Kket);
-    a.o_bar = o; o += 2 * MD_HL_STAGES;
-    a.o_r0 = o; o += nR * a.rs0;
-    a.o_g0 = o; o += even_up(nR * (L + 1));
-    a.o_pq = o; o += even_up(nR * 3);
-    o = up16(o);
-    a.o_ov = o; o += a.ov_doubles;
-    a.o_ring = o; o += MD_HL_STAGES * a.ring_stage;
-    a.total = o;
-    P.smem = (size_t)o * 8;
-    if (P.smem > (size_t)g_hl_max_smem) return false;
+    const int t1_b = c.pure ? ncart(a.la) * 20 : 0, t1_k = c.pure ? ncart(a.lc) * 20 : 0;    // T1 rows of 20 doubles (hl.cuh)
+    const int s1_need = std::max(3 * esz_b + 1 + 8 * t1_b, 3 * esz_k + 1 + 8 * t1_k);
+    bool fits = false;
+    for (int kc2 = 16; kc2 >= 8 && !fits; kc2 -= 8) {     // 16 stacked rows per GEMM2 chunk when shared memory allows
+        a.kc2 = kc2;
+        a.mrows_pad = (a.mrows + kc2 - 1) / kc2 * kc2;
+        a.ring_stage = up16(std::max(MD_HL_KC1 * NTS, kc2 * a.sb));
+        int ov = std::max(a.mrows_pad * NTS, nR * a.rs1);
+        ov = std::max(ov, s1_need - MD_HL_STAGES * a.ring_stage);
+        a.ov_doubles = up16(ov);
+        int o = 0;
+        a.o_herm = o; o += even_up(nherm(std::max(a.Lb, a.Lk))) / 2 + 1;
+        a.o_rowinfo = o; o += a.mrows_pad;
+        a.o_ct = o; o += 4 * 28 * MD_HL_CSTR;
+        a.o_hdr = o; o += 4 * (a.Kbra + a.Kket);
+        a.o_bar = o; o += 2 * MD_HL_STAGES;
+        a.o_r0 = o; o += nR * a.rs0;
+        a.o_g0 = o; o += even_up(nR * (L + 1));
+        a.o_pq = o; o += even_up(nR * 3);
+        o = up16(o);
+        a.o_ov = o; o += a.ov_doubles;
+        a.o_ring = o; o += MD_HL_STAGES * a.ring_stage;
+        o += 128;                                          // fragment loads of row tiles past the end stay inside the allocation
+        a.total = o;
+        P.smem = (size_t)o * 8;
+        fits = P.smem <= (size_t)g_hl_max_smem;
+    }
+    if (!fits) return false;
+    P.npass = (a.mrows_pad / 8 + warps * MW - 1) / (warps * MW);
     if (!hl_table()[((warps == 8) * 5 + MW) * 5 + NW]) return false;
 
     const long long hb_doubles = (long long)a.mrows_pad * a.sb;
     const long long hk_doubles = (long long)a.ntile * a.Kket * a.nhk_pad * NTS;
     a.off_hk = (hb_doubles + 15) / 16 * 16;
     a.scratch_stride = (a.off_hk + hk_doubles + 15) / 16 * 16;
-    const int by_regs = warps == 4 ? 3 : (MW <= 2 ? 2 : 1);
+    const int by_regs = warps == 4 ? 3 : 1;             // __launch_bounds__ of hl_kernel
     P.ctas = (int)std::max<size_t>(1, std::min<size_t>(by_regs, (size_t)(g_hl_max_smem + 1024) / (P.smem + 1024)));
     P.grid = (unsigned)std::min<long long>(c.nq, (long long)nsm * P.ctas);
     P.scratch_bytes = (size_t)P.grid * a.scratch_stride * 8;

@@ -467,7 +467,10 @@ int md_fp64_peak(int kind, int seconds_x10, double *tflops, double *ms_out) {
     cudaEvent_t e0, e1;
     CK(cudaEventCreate(&e0));
     CK(cudaEventCreate(&e1));
-    const int blocks = S.nsm * 8, threads = 256;
+    // MD_PEAK_SHAPE="blocks_per_sm,threads" (measurement only): occupancy dependence of the issue loops
+    int bps = 8, threads = 256;
+    if (const char *f = getenv("MD_PEAK_SHAPE")) sscanf(f, "%d,%d", &bps, &threads);
+    const int blocks = S.nsm * bps;
     int iters = 4096;
     double flop_per_iter = kind == 0 ? 2.0 * 16 * threads * blocks
                          : kind == 1 ? 512.0 * 8 * (threads / 32) * blocks

@@ -7,7 +7,7 @@
 namespace mdb {
 
 // 16 independent FMA chains per thread; 2*16*iters flop per thread.
-__global__ void __launch_bounds__(256) peak_dfma_kernel(double *out, int iters, double a, double b) {
+__global__ void __launch_bounds__(1024) peak_dfma_kernel(double *out, int iters, double a, double b) {
     double x[16];
 #pragma unroll
     for (int i = 0; i < 16; ++i) x[i] = threadIdx.x * 1e-3 + i;
@@ -22,7 +22,7 @@ __global__ void __launch_bounds__(256) peak_dfma_kernel(double *out, int iters, 
 }
 
 // 8 independent m8n8k4 accumulators per warp; 512 flop per mma per warp.
-__global__ void __launch_bounds__(256) peak_dmma_kernel(double *out, int iters, double a, double b) {
+__global__ void __launch_bounds__(1024) peak_dmma_kernel(double *out, int iters, double a, double b) {
     double c[8][2];
 #pragma unroll
     for (int i = 0; i < 8; ++i) { c[i][0] = threadIdx.x * 1e-3; c[i][1] = i; }
@@ -39,7 +39,7 @@ __global__ void __launch_bounds__(256) peak_dmma_kernel(double *out, int iters, 
 }
 
 // 4 independent m16n8k8 accumulators per warp (sm_90+ shape); 2*16*8*8 = 2048 flop per mma.
-__global__ void __launch_bounds__(256) peak_dmma16_kernel(double *out, int iters, double a, double b) {
+__global__ void __launch_bounds__(1024) peak_dmma16_kernel(double *out, int iters, double a, double b) {
     double c[4][4];
 #pragma unroll
     for (int i = 0; i < 4; ++i) { c[i][0] = threadIdx.x * 1e-3; c[i][1] = i; c[i][2] = 1; c[i][3] = 2; }
@@ -58,7 +58,7 @@ __global__ void __launch_bounds__(256) peak_dmma16_kernel(double *out, int iters
 
 // Mixed: even warps run the DFMA chains, odd warps the m8n8k4 DMMA chains, same iteration count.  If the vector and
 // tensor FP64 paths were separate units the sum would exceed either peak; on B200 it does not.
-__global__ void __launch_bounds__(256) peak_mixed_kernel(double *out, int iters, double a, double b) {
+__global__ void __launch_bounds__(1024) peak_mixed_kernel(double *out, int iters, double a, double b) {
     double s = 0;
     if ((threadIdx.x >> 5) & 1) {
         double c[8][2];
