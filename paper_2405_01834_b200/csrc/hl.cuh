@@ -40,7 +40,13 @@ struct HlArgs {
     int sb;                              // row stride of Hb in the scratch: >= 8*ceil(nab/8), = 4 mod 16
     int ntile;                           // cd tiles
     int q_first;                         // first GEMM1 chunk row with a non-zero Hk (one-centre solid kets), multiple of KC1
-    double *scratch;                     // [grid][scratch_stride]
+    double *scratch;                     // fused mode: [grid][scratch_stride]
+    int fused;                           // 1: S1 runs inside the quartet kernel into the CTA's scratch; 0: pair records
+    int by_quartet;                      // record mode: 1 = record r belongs to quartet q_begin + r, 0 = to pair r
+    const double *rec_b, *rec_k;         // record mode: H records of hl_pair_kernel (same layout as the scratch halves)
+    const double *hdr_b, *hdr_k;         // record mode: {p, Px, Py, Pz} per record and primitive
+    long long rec_stride_b, rec_stride_k;
+    long long q_begin, q_end;            // quartets of this launch
     long long scratch_stride, off_hk;    // doubles per CTA; offset of the ket part
     const int32_t *qidx;
     long long nq, nket;
@@ -174,7 +180,11 @@ __device__ __forceinline__ void hl_build_H(int la, int lb, int pure, bool neg, d
     constexpr int NWARPS = NTHR / 32, TS = 20;              // T1 row stride: 16 columns + 4 (conflict-free fragments)
     const int ntb = (nsb + 7) >> 3, nta = (nsa + 7) >> 3;   // column tiles of mb, row tiles of ma (1 or 2)
     const int ksb = (ncb + 3) >> 2, ksa = (nca + 3) >> 2;   // K steps over b and over a (<= 7)
-    const int pchunk = max(1, min(nh, t1cap / (nca * TS)));
+    // A warp owns groups of pw consecutive Hermite rows end to end (stage A into its private T1 slice, stage B out of
+    // it), so the loop has no CTA barrier: the LDS-bound stage A of one warp overlaps the tensor-core steps of the others.
+    const int pw = nca >= 21 ? 1 : nca >= 10 ? 2 : nca >= 6 ? 4 : 8;      // pw * nca rows: a multiple of 8, or nearly
+    double *T1w = T1 + (size_t)warp * pw * nca * TS;                       // needs t1cap >= NWARPS * pw * nca * TS (host)
+    (void)t1cap;
     double cbf[7][2], caf[7][2];                            // constant fragments: C^{lb}[b][mb], C^{la}[a][ma]
     uint32_t boff[7];                                       // per K step: offsets bx*nt | by*nt << 8 | bz*nt << 16 of b = 4k + lc
 #pragma unroll
@@ -189,10 +199,10 @@ __device__ __forceinline__ void hl_build_H(int la, int lb, int pure, bool neg, d
             caf[k][n] = b < nca ? CaT[b * MD_HL_CSTR + 8 * n + lr] : 0.0;    // same lane pattern: a = 4k + lc, ma = 8n + lr
         }
     }
-    for (int h0 = 0; h0 < nh; h0 += pchunk) {
-        const int hc = min(pchunk, nh - h0);
+    for (int h0 = warp * pw; h0 < nh; h0 += NWARPS * pw) {
+        const int hc = min(pw, nh - h0);
         const int nrows = hc * nca, nmt = (nrows + 7) >> 3;
-        for (int mt = warp; mt < nmt; mt += NWARPS) {
+        for (int mt = 0; mt < nmt; ++mt) {
             const int r = mt * 8 + lr;
             const bool rv = r < nrows;
             const int rr = rv ? r : nrows - 1;
@@ -201,7 +211,7 @@ __device__ __forceinline__ void hl_build_H(int la, int lb, int pure, bool neg, d
             unpack_tuv(s_herm[h0 + ih], t, u, v);
             unpack_tuv(ca[a], ax, ay, az);
             const double *ex = Ex + ax * (lb + 1) * nt + t, *ey = Ey + ay * (lb + 1) * nt + u, *ez = Ez + az * (lb + 1) * nt + v;
-            double c[2][2] = {{0.0, 0.0}, {0.0, 0.0}};
+            double c[2][2] = {{0.0, 0.0}, {0.0, 0.0}}, d[2][2] = {{0.0, 0.0}, {0.0, 0.0}};   // even / odd K steps: two chains
             // all operands first (21 loads in flight), then the votes, then the tensor-core steps
             double x[7];
             uint32_t live = 0;
@@ -216,19 +226,25 @@ __device__ __forceinline__ void hl_build_H(int la, int lb, int pure, bool neg, d
 #pragma unroll
             for (int k = 0; k < 7; ++k) {
                 if (live >> k & 1) {
-                    hl_dmma884(c[0][0], c[0][1], x[k], cbf[k][0]);
-                    if (ntb > 1) hl_dmma884(c[1][0], c[1][1], x[k], cbf[k][1]);
+                    if (k & 1) {
+                        hl_dmma884(d[0][0], d[0][1], x[k], cbf[k][0]);
+                        if (ntb > 1) hl_dmma884(d[1][0], d[1][1], x[k], cbf[k][1]);
+                    } else {
+                        hl_dmma884(c[0][0], c[0][1], x[k], cbf[k][0]);
+                        if (ntb > 1) hl_dmma884(c[1][0], c[1][1], x[k], cbf[k][1]);
+                    }
                 }
             }
-            double *o = T1 + (size_t)r * TS + 2 * lc;
+            c[0][0] += d[0][0]; c[0][1] += d[0][1]; c[1][0] += d[1][0]; c[1][1] += d[1][1];
+            double *o = T1w + (size_t)r * TS + 2 * lc;
             if (rv) {
                 *(double2 *)o = make_double2(c[0][0], c[0][1]);
                 if (ntb > 1) *(double2 *)(o + 8) = make_double2(c[1][0], c[1][1]);
             }
         }
-        __syncthreads();
-        for (int ih = warp; ih < hc; ih += NWARPS) {
-            const double *t1 = T1 + (size_t)ih * nca * TS + lr;
+        __syncwarp();
+        for (int ih = 0; ih < hc; ++ih) {
+            const double *t1 = T1w + (size_t)ih * nca * TS + lr;
             double c[2][2][2] = {{{0.0, 0.0}, {0.0, 0.0}}, {{0.0, 0.0}, {0.0, 0.0}}};      // [ma tile][mb tile][2]
             double b0[7], b1[7];
             uint32_t live = 0;
@@ -263,8 +279,9 @@ __device__ __forceinline__ void hl_build_H(int la, int lb, int pure, bool neg, d
                     if (ma < nsa && mb + 1 < nsb) *dst(h0 + ih, ma * nsb + mb + 1) = sgn * c[i][n][1];
                 }
         }
-        __syncthreads();
+        __syncwarp();                                       // the slice is rewritten by the warp's next group
     }
+    __syncthreads();
 }
 
 // One K step (4 ket Hermite rows) of GEMM1 for a warp's MW x NW tiles: the A elements [p~+q~]^(0) are gathered from
@@ -283,6 +300,110 @@ __device__ __forceinline__ void hl_gemm1_step(double (&acc)[MW][NW][2], const do
 #pragma unroll
         for (int n = 0; n < NW; ++n)
             if (FULLN || n < nnt) hl_dmma884(acc[i][n][0], acc[i][n][1], a[i], bfr[n]);
+}
+
+// ---- S1 for one side of one quartet (or one shell pair): every primitive pair's Hermite tables (three warps, one
+// per axis), {p, P} header and dense H record.  ws = shared scratch of cap doubles.  rec: bra [K][nh][sb], ket
+// [cd tile][K][nh_pad][NT+4] (tile_stride = K nh_pad (NT+4)).  Ends with a barrier.
+template <int NTHR, int NT>
+__device__ __forceinline__ void hl_side(const PairView &pv, bool ket, int l1, int l2, int K1, int K2, int pure, long long ip,
+                                        double *hdr, double *ws, int cap, const uint32_t *s_herm, const double *CaT,
+                                        const double *CbT, double *rec, int nh, int nh_pad, int sb, long long tile_stride) {
+    const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+    long long i1 = ip, i2 = ip;
+    if (pv.idx) { i1 = pv.idx[2 * ip]; i2 = pv.idx[2 * ip + 1]; }
+    const int esz = (l1 + 1) * (l2 + 1) * (l1 + l2 + 1);
+    double *E = ws, *T1 = ws + ((3 * esz + 1) & ~1);               // 16-byte aligned rows for the fragment stores
+    const int t1cap = cap - ((3 * esz + 1) & ~1);
+    for (int kp = 0; kp < K1 * K2; ++kp) {
+        const int k1 = kp / K2, k2 = kp - k1 * K2;
+        const double za = pv.a.exps[i1 * K1 + k1];
+        const double zb = pv.single ? 0.0 : pv.b.exps[i2 * K2 + k2];
+        const double coef = pv.a.coefs[i1 * K1 + k1] * (pv.single ? 1.0 : pv.b.coefs[i2 * K2 + k2]);
+        if (warp < 3) {
+            const double A = pv.a.center[3 * i1 + warp], B = pv.single ? A : pv.b.center[3 * i2 + warp];
+            hl_e_axis_warp(l1, l2, za, zb, A - B, E + warp * esz, lane);
+            if (lane == 0) {
+                double *h = hdr + 4 * kp;
+                h[1 + warp] = (za * A + zb * B) / (za + zb);
+                if (warp == 0) h[0] = za + zb;
+            }
+        }
+        __syncthreads();
+        if (pv.single && pure) {
+            // One-centre solid harmonics (Hobson): S_lm(d/dA) e^{-z r_A^2} = (2z)^l S_lm(r_A) e^{-z r_A^2}: only the
+            // Hermites of order exactly l appear, with coefficient C^l_{m,q~}/(2z)^l; lower rows are exact zeros.
+            const int ns = nsolid(l1), nlow = nherm(l1 - 1);
+            double f = coef;
+            for (int i = 0; i < l1; ++i) f *= 0.5 / za;
+            if (l1 & 1) f = -f;
+            HlKetDst<NT> dst{rec + (long long)kp * nh_pad * (NT + 4), tile_stride};
+            for (int e = tid; e < nh * ns; e += NTHR) {
+                const int ih = e / ns, m = e - ih * ns;
+                *dst(ih, m) = ih < nlow ? 0.0 : f * CaT[(ih - nlow) * MD_HL_CSTR + m];
+            }
+            __syncthreads();
+        } else if (ket) {
+            HlKetDst<NT> dst{rec + (long long)kp * nh_pad * (NT + 4), tile_stride};
+            hl_build_H<NTHR>(l1, l2, pure, true, coef, E, T1, t1cap, s_herm, CaT, CbT, dst);
+        } else {
+            HlBraDst dst{rec + (long long)kp * nh * sb, sb};
+            hl_build_H<NTHR>(l1, l2, pure, false, coef, E, T1, t1cap, s_herm, CaT, CbT, dst);
+        }
+    }
+}
+
+// Constant tables of a CTA: Hermite triples and the transposed, zero-padded Cartesian->solid tables of up to 4 shells.
+template <int NTHR>
+__device__ __forceinline__ void hl_stage_tables(uint32_t *s_herm, int nhm, double *CT, const int (&ls)[4]) {
+    const int tid = threadIdx.x, CTS = 28 * MD_HL_CSTR;
+    for (int i = tid; i < nhm; i += NTHR) s_herm[i] = c_herm[i];
+    for (int i = tid; i < 4 * CTS; i += NTHR) CT[i] = 0.0;
+    __syncthreads();
+    for (int s = 0; s < 4; ++s) {
+        const int l = ls[s], nc = ncart(l), ns = nsolid(l);
+        for (int i = tid; i < nc * ns; i += NTHR) {
+            const int m = i / nc, c = i - m * nc;
+            CT[s * CTS + c * MD_HL_CSTR + m] = c_solid[solid_off(l) + i];
+        }
+    }
+}
+
+// ---- S1 as a kernel of its own: one H record per CTA iteration (per shell pair, or per quartet side), for the record
+// mode of hl_kernel.  Persistent 4-warp CTAs, several per SM.
+struct HlPairArgs {
+    PairView pv;
+    int ket, l1, l2, K1, K2, pure;
+    int nh, nh_pad, sb;
+    long long tile_stride;
+    long long nrec, rec_stride;
+    double *rec, *hdr;                   // [nrec][rec_stride], [nrec][K1*K2][4]
+    int by_quartet;                      // record r <- side of quartet q_begin + r instead of pair r
+    const int32_t *qidx;
+    long long q_begin, nket;
+    int o_herm, o_ct, o_ws, ws_doubles;  // shared-memory carve-up (doubles)
+};
+
+template <int NW>
+__global__ void __launch_bounds__(128, 4) hl_pair_kernel(HlPairArgs g) {
+    constexpr int NTHR = 128, NT = 8 * NW;
+    extern __shared__ double sm[];
+    uint32_t *s_herm = (uint32_t *)(sm + g.o_herm);
+    double *CT = sm + g.o_ct;
+    const int ls[4] = {g.l1, g.l2, 0, 0};
+    hl_stage_tables<NTHR>(s_herm, nherm(g.l1 + g.l2), CT, ls);
+    __syncthreads();
+    for (long long r = blockIdx.x; r < g.nrec; r += gridDim.x) {
+        long long ip = r;
+        if (g.by_quartet) {
+            const long long q = g.q_begin + r;
+            if (g.qidx) ip = g.qidx[2 * q + g.ket];
+            else ip = g.ket ? q % g.nket : q / g.nket;
+        }
+        hl_side<NTHR, NT>(g.pv, g.ket != 0, g.l1, g.l2, g.K1, g.K2, g.pure, ip, g.hdr + r * 4 * g.K1 * g.K2, sm + g.o_ws,
+                          g.ws_doubles, s_herm, CT, CT + 28 * MD_HL_CSTR, g.rec + r * g.rec_stride, g.nh, g.nh_pad, g.sb,
+                          g.tile_stride);
+    }
 }
 
 // Order in which one quartet's H chunks pass through the ring: for every cd tile, for every row pass of GEMM1 the
@@ -310,8 +431,8 @@ __global__ void __launch_bounds__(32 * NWARPS, (NWARPS == 4 ? 3 : 1)) hl_kernel(
     const int L = g.Lb + g.Lk, nhb = g.nhb, nhk = g.nhk;
     const uint2 *lut = (const uint2 *)g.rlut;
     const int CTS = 28 * MD_HL_CSTR;
-    double *scr = g.scratch + (long long)blockIdx.x * g.scratch_stride;
-    double *hb = scr, *hk = scr + g.off_hk;
+    double *scr = g.fused ? g.scratch + (long long)blockIdx.x * g.scratch_stride : nullptr;
+    const double *hb = scr, *hk = scr ? scr + g.off_hk : nullptr;   // fused mode; record mode sets them per quartet
     const int nmt = g.mrows_pad >> 3, npass = (nmt + NWARPS * MW - 1) / (NWARPS * MW);
     const int nc1 = g.nhk_pad / MD_HL_KC1, c_first = g.q_first / MD_HL_KC1, nc2 = g.mrows_pad / g.kc2;
     const int nmt2 = (g.nab + 7) >> 3;
@@ -320,18 +441,8 @@ __global__ void __launch_bounds__(32 * NWARPS, (NWARPS == 4 ? 3 : 1)) hl_kernel(
 
     // ---- once per CTA: constant tables, barriers, zeroed scratch (its padding is never written again) ----
     {
-        const int nhm = nherm(max(g.Lb, g.Lk));
-        for (int i = tid; i < nhm; i += NTHR) s_herm[i] = c_herm[i];
         const int ls[4] = {g.la, g.lb, g.lc, g.ld};
-        for (int i = tid; i < 4 * CTS; i += NTHR) CT[i] = 0.0;
-        __syncthreads();
-        for (int s = 0; s < 4; ++s) {
-            const int l = ls[s], nc = ncart(l), ns = nsolid(l);
-            for (int i = tid; i < nc * ns; i += NTHR) {
-                const int m = i / nc, c = i - m * nc;
-                CT[s * CTS + c * MD_HL_CSTR + m] = c_solid[solid_off(l) + i];
-            }
-        }
+        hl_stage_tables<NTHR>(s_herm, nherm(max(g.Lb, g.Lk)), CT, ls);
         for (int r = tid; r < g.mrows_pad; r += NTHR) {
             const int rr = min(r, g.mrows - 1), kb = rr / nhb;
             rowinfo[r] = make_int2((int)c_herm[rr - kb * nhb], kb);
@@ -340,7 +451,7 @@ __global__ void __launch_bounds__(32 * NWARPS, (NWARPS == 4 ? 3 : 1)) hl_kernel(
             for (int s = 0; s < ST; ++s) { hl_bar_init(full + s, 1); hl_bar_init(empty + s, NWARPS); }
             asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
         }
-        for (long long i = tid; i < g.scratch_stride; i += NTHR) scr[i] = 0.0;
+        if (g.fused) for (long long i = tid; i < g.scratch_stride; i += NTHR) scr[i] = 0.0;
     }
     long long gcons = 0, gprod = 0;                        // chunks consumed (all threads) / issued (thread 0), CTA lifetime
     HlStream ps;
@@ -377,61 +488,26 @@ __global__ void __launch_bounds__(32 * NWARPS, (NWARPS == 4 ? 3 : 1)) hl_kernel(
         if (tid == 0 && left > 0) produce();
     };
 
-    for (long long q = blockIdx.x; q < g.nq; q += gridDim.x) {
+    for (long long q = g.q_begin + blockIdx.x; q < g.q_end; q += gridDim.x) {
         long long bi, ki;
         if (g.qidx) { bi = g.qidx[2 * q]; ki = g.qidx[2 * q + 1]; }
         else { bi = q / g.nket; ki = q % g.nket; }
         double *out = g.out + q * g.s_q + bi * g.s_bi + ki * g.s_ki;
         __syncthreads();                                   // the previous quartet is done with shared memory and the scratch
 
-        // ---- S1: Hermite tables and H of every primitive pair of both sides -> scratch ----
-        for (int side = 0; side < 2; ++side) {
-            const PairView &pv = side ? g.ket : g.bra;
-            const int l1 = side ? g.lc : g.la, l2 = side ? g.ld : g.lb;
-            const int K1 = side ? g.Kc : g.Ka, K2 = side ? g.Kd : g.Kb;
-            const long long ip = side ? ki : bi;
-            long long i1 = ip, i2 = ip;
-            if (pv.idx) { i1 = pv.idx[2 * ip]; i2 = pv.idx[2 * ip + 1]; }
-            const int esz = (l1 + 1) * (l2 + 1) * (l1 + l2 + 1);
-            double *E = ov, *T1 = ov + ((3 * esz + 1) & ~1);           // 16-byte aligned rows for the fragment stores
-            const int t1cap = g.ov_doubles + ST * g.ring_stage - ((3 * esz + 1) & ~1);
-            for (int kp = 0; kp < K1 * K2; ++kp) {
-                const int k1 = kp / K2, k2 = kp - k1 * K2;
-                const double za = pv.a.exps[i1 * K1 + k1];
-                const double zb = pv.single ? 0.0 : pv.b.exps[i2 * K2 + k2];
-                const double coef = pv.a.coefs[i1 * K1 + k1] * (pv.single ? 1.0 : pv.b.coefs[i2 * K2 + k2]);
-                if (warp < 3) {
-                    const double A = pv.a.center[3 * i1 + warp], B = pv.single ? A : pv.b.center[3 * i2 + warp];
-                    hl_e_axis_warp(l1, l2, za, zb, A - B, E + warp * esz, lane);
-                    if (lane == 0) {
-                        double *h = hdr + 4 * ((side ? g.Kbra : 0) + kp);
-                        h[1 + warp] = (za * A + zb * B) / (za + zb);
-                        if (warp == 0) h[0] = za + zb;
-                    }
-                }
-                __syncthreads();
-                const double *CaT = CT + (side ? 2 : 0) * CTS, *CbT = CT + (side ? 3 : 1) * CTS;
-                if (pv.single && g.pure) {
-                    // One-centre solid harmonics (Hobson): S_lm(d/dA) e^{-z r_A^2} = (2z)^l S_lm(r_A) e^{-z r_A^2}: only the
-                    // Hermites of order exactly l appear, with coefficient C^l_{m,q~}/(2z)^l; lower rows are exact zeros.
-                    const int ns = nsolid(l1), nlow = nherm(l1 - 1);
-                    double f = coef;
-                    for (int i = 0; i < l1; ++i) f *= 0.5 / za;
-                    if (l1 & 1) f = -f;
-                    HlKetDst<NT> dst{hk + (long long)kp * g.nhk_pad * NTS, hk_tile};
-                    for (int e = tid; e < nhk * ns; e += NTHR) {
-                        const int ih = e / ns, m = e - ih * ns;
-                        *dst(ih, m) = ih < nlow ? 0.0 : f * CaT[(ih - nlow) * MD_HL_CSTR + m];
-                    }
-                    __syncthreads();
-                } else if (side) {
-                    HlKetDst<NT> dst{hk + (long long)kp * g.nhk_pad * NTS, hk_tile};
-                    hl_build_H<NTHR>(l1, l2, g.pure, true, coef, E, T1, t1cap, s_herm, CaT, CbT, dst);
-                } else {
-                    HlBraDst dst{hb + (long long)kp * nhb * g.sb, g.sb};
-                    hl_build_H<NTHR>(l1, l2, g.pure, false, coef, E, T1, t1cap, s_herm, CaT, CbT, dst);
-                }
-            }
+        // ---- S1: Hermite tables and H of every primitive pair of both sides -> scratch (fused mode), or the records ----
+        if (g.fused) {
+            const int cap = g.ov_doubles + ST * g.ring_stage;
+            hl_side<NTHR, NT>(g.bra, false, g.la, g.lb, g.Ka, g.Kb, g.pure, bi, hdr, ov, cap, s_herm, CT, CT + CTS, scr,
+                              nhb, 0, g.sb, 0);
+            hl_side<NTHR, NT>(g.ket, true, g.lc, g.ld, g.Kc, g.Kd, g.pure, ki, hdr + 4 * g.Kbra, ov, cap, s_herm, CT + 2 * CTS,
+                              CT + 3 * CTS, scr + g.off_hk, nhk, g.nhk_pad, 0, hk_tile);
+        } else {
+            const long long rb = g.by_quartet ? q - g.q_begin : bi, rk = g.by_quartet ? q - g.q_begin : ki;
+            hb = g.rec_b + rb * g.rec_stride_b;
+            hk = g.rec_k + rk * g.rec_stride_k;
+            for (int i = tid; i < 4 * (g.Kbra + g.Kket); i += NTHR)
+                hdr[i] = i < 4 * g.Kbra ? g.hdr_b[rb * 4 * g.Kbra + i] : g.hdr_k[rk * 4 * g.Kket + i - 4 * g.Kbra];
         }
         __threadfence();
         asm volatile("fence.proxy.async;" ::: "memory");   // generic-proxy stores to the scratch before the bulk copies read it

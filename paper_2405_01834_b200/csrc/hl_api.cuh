@@ -20,7 +20,8 @@ cudaError_t hl_init(int max_smem, const uint32_t *herm, const double *solid);
 // (it then falls to the runtime-l chain), else 1 and the scratch the launch needs in *scratch_bytes.
 int hl_plan(const HlCall &c, int nsm, size_t *scratch_bytes);
 // Launch with the plan of the same call; scratch = device buffer of *scratch_bytes.  info (may be null) receives
-// {MW, NW, warps, smem bytes, CTAs per SM, row passes, cd tiles, grid}.
-cudaError_t hl_launch(const HlCall &c, int nsm, void *scratch, cudaStream_t st, int *info);
+// {MW, NW, warps, smem bytes, CTAs per SM, row passes, S1 mode (0 in-kernel, 1 per pair, 2 per quartet chunk), grid};
+// launches = kernels enqueued.
+cudaError_t hl_launch(const HlCall &c, int nsm, void *scratch, cudaStream_t st, int *info, int *launches);
 
 }  // namespace mdb

@@ -10,9 +10,11 @@ namespace mdb {
 
 namespace {
 HlFn g_hl[2][5][5];                   // [0]: 4 warps, [1]: 8 warps; [MW][NW]
+HlPairFn g_hl_pair[5];                // [NW]
 int g_hl_max_smem = 227 * 1024;
 }  // namespace
 HlFn *hl_table() { return &g_hl[0][0][0]; }
+HlPairFn *hl_pair_table() { return g_hl_pair; }
 
 cudaError_t hl_init(int max_smem, const uint32_t *herm, const double *solid) {
     g_hl_max_smem = max_smem;
@@ -28,6 +30,11 @@ struct HlPlan {
     int MW, NW, warps, ctas, npass;
     size_t smem, scratch_bytes;
     unsigned grid;
+    int mode;                             // 0 fused (S1 in the quartet kernel), 1 records per shell pair, 2 records per quartet, in chunks
+    long long chunk;                      // quartets per launch (mode 2)
+    long long recb, reck;                 // doubles per record
+    HlPairArgs pb, pk;
+    size_t pair_smem_b, pair_smem_k;
 };
 
 inline int even_up(int x) { return x + (x & 1); }
@@ -58,8 +65,14 @@ bool make_plan(const HlCall &c, int nsm, HlPlan &P) {
     const int ntile = (nnt_total + 3) / 4;
     int NW = (nnt_total + ntile - 1) / ntile;
     int warps, MW;
-    if (nmt <= 12 && nmt2 <= 4 * MD_HL_MT2) { warps = 4; MW = std::min(3, (nmt + 3) / 4); }
-    else { warps = 8; MW = std::min(4, (nmt + 7) / 8); }
+    // By measurement (profiles/r02_hl_tune.md): 4-warp CTAs (three per SM) for the small classes, else 8 warps; the row tiles
+    // per warp that give the fewest tile slots over all row passes, the larger on ties.
+    warps = (nmt <= 12 && nmt2 <= 4 * MD_HL_MT2) ? 4 : 8;
+    MW = 1;
+    for (int m = 1, best = 1 << 30; m <= (warps == 4 ? 3 : 4); ++m) {
+        const int slots = (nmt + warps * m - 1) / (warps * m) * m;
+        if (slots <= best) { best = slots; MW = m; }
+    }
     if (const char *f = getenv("MD_HL_FORCE")) {           // measurement override: "MW,NW,warps"
         int m, n, w;
         if (sscanf(f, "%d,%d,%d", &m, &n, &w) == 3 && (w == 4 || w == 8) && m >= 1 && m <= (w == 4 ? 3 : 4) && n >= 1 && n <= 4) {
@@ -72,8 +85,9 @@ bool make_plan(const HlCall &c, int nsm, HlPlan &P) {
     P.MW = MW; P.NW = NW; P.warps = warps;
 
     const int esz_b = (a.la + 1) * (a.lb + 1) * (a.Lb + 1), esz_k = (a.lc + 1) * (a.ld + 1) * (a.Lk + 1);
-    const int t1_b = c.pure ? ncart(a.la) * 20 : 0, t1_k = c.pure ? ncart(a.lc) * 20 : 0;    // T1 rows of 20 doubles (hl.cuh)
-    const int s1_need = std::max(3 * esz_b + 1 + 8 * t1_b, 3 * esz_k + 1 + 8 * t1_k);
+    auto t1_slice = [](int l) { const int nc = ncart(l); return (nc >= 21 ? 1 : nc >= 10 ? 2 : nc >= 6 ? 4 : 8) * nc * 20; };   // hl_build_H
+    const int t1_b = c.pure ? t1_slice(a.la) : 0, t1_k = c.pure ? t1_slice(a.lc) : 0;
+    const int s1_need = std::max(3 * esz_b + 2 + warps * t1_b, 3 * esz_k + 2 + warps * t1_k);
     bool fits = false;
     for (int kc2 = 16; kc2 >= 8 && !fits; kc2 -= 8) {     // 16 stacked rows per GEMM2 chunk when shared memory allows
         a.kc2 = kc2;
@@ -107,10 +121,55 @@ bool make_plan(const HlCall &c, int nsm, HlPlan &P) {
     const long long hk_doubles = (long long)a.ntile * a.Kket * a.nhk_pad * NTS;
     a.off_hk = (hb_doubles + 15) / 16 * 16;
     a.scratch_stride = (a.off_hk + hk_doubles + 15) / 16 * 16;
+    P.recb = a.off_hk; P.reck = (hk_doubles + 15) / 16 * 16;
     const int by_regs = warps == 4 ? 3 : 1;             // __launch_bounds__ of hl_kernel
     P.ctas = (int)std::max<size_t>(1, std::min<size_t>(by_regs, (size_t)(g_hl_max_smem + 1024) / (P.smem + 1024)));
     P.grid = (unsigned)std::min<long long>(c.nq, (long long)nsm * P.ctas);
-    P.scratch_bytes = (size_t)P.grid * a.scratch_stride * 8;
+
+    // Where S1 runs: per shell pair when the pair records fit the budget and pairs are shared by
+    // quartets; else per quartet side, in chunks of quartets that fit the budget; else inside the quartet kernel.
+    size_t budget = (size_t)2048 << 20;
+    if (const char *f = getenv("MD_HL_WS_MB")) budget = (size_t)atoll(f) << 20;
+    int mode = -1;
+    if (const char *f = getenv("MD_HL_MODE")) mode = atoi(f);
+    const long long npb = c.bra.npairs, npk = c.ket.npairs;
+    const size_t per_pair = 8 * ((size_t)npb * (P.recb + 4 * a.Kbra) + (size_t)npk * (P.reck + 4 * a.Kket));
+    const size_t per_quartet = 8 * (size_t)(P.recb + P.reck + 4 * (a.Kbra + a.Kket));
+    if (mode < 0) {
+        if (per_pair <= budget && npb + npk <= 2 * c.nq) mode = 1;
+        else if (per_quartet * P.grid <= budget) mode = 2;
+        else mode = 0;
+    }
+    if (mode == 1 && per_pair > budget) mode = 2;
+    if (mode == 2 && per_quartet * P.grid > budget) mode = 0;
+    P.mode = mode;
+    a.fused = mode == 0; a.by_quartet = mode == 2;
+    a.rec_stride_b = P.recb; a.rec_stride_k = P.reck;
+    P.chunk = c.nq;
+    if (mode == 0) P.scratch_bytes = (size_t)P.grid * a.scratch_stride * 8;
+    else if (mode == 1) P.scratch_bytes = per_pair;
+    else {
+        P.chunk = std::min<long long>(c.nq, (long long)(budget / per_quartet) / P.grid * P.grid);
+        P.scratch_bytes = (size_t)P.chunk * per_quartet;
+    }
+    for (int side = 0; side < 2 && mode; ++side) {
+        HlPairArgs &g = side ? P.pk : P.pb;
+        g.pv = side ? c.ket : c.bra; g.ket = side;
+        g.l1 = side ? a.lc : a.la; g.l2 = side ? a.ld : a.lb; g.K1 = side ? a.Kc : a.Ka; g.K2 = side ? a.Kd : a.Kb;
+        g.pure = c.pure; g.nh = side ? a.nhk : a.nhb; g.nh_pad = side ? a.nhk_pad : 0; g.sb = side ? 0 : a.sb;
+        g.tile_stride = side ? (long long)a.Kket * a.nhk_pad * NTS : 0;
+        g.rec_stride = side ? P.reck : P.recb;
+        g.by_quartet = mode == 2; g.qidx = c.qidx; g.nket = npk;
+        const int esz = (g.l1 + 1) * (g.l2 + 1) * (g.l1 + g.l2 + 1);
+        int o = 0;
+        g.o_herm = o; o += nherm(g.l1 + g.l2) / 2 + 1;
+        g.o_ct = o; o += 4 * 28 * MD_HL_CSTR;
+        o = up16(o);
+        g.o_ws = o;
+        g.ws_doubles = 3 * esz + 2 + (c.pure ? 4 * t1_slice(g.l1) : 0);                      // 4 warps (hl_pair_kernel)
+        o += g.ws_doubles;
+        (side ? P.pair_smem_k : P.pair_smem_b) = (size_t)o * 8;
+    }
     return true;
 }
 
@@ -123,14 +182,46 @@ int hl_plan(const HlCall &c, int nsm, size_t *scratch_bytes) {
     return 1;
 }
 
-cudaError_t hl_launch(const HlCall &c, int nsm, void *scratch, cudaStream_t st, int *info) {
+cudaError_t hl_launch(const HlCall &c, int nsm, void *scratch, cudaStream_t st, int *info, int *launches) {
     HlPlan P;
     if (!make_plan(c, nsm, P)) return cudaErrorInvalidConfiguration;
-    P.a.scratch = (double *)scratch;
-    hl_table()[((P.warps == 8) * 5 + P.MW) * 5 + P.NW]<<<P.grid, 32 * P.warps, P.smem, st>>>(P.a);
+    HlFn fn = hl_table()[((P.warps == 8) * 5 + P.MW) * 5 + P.NW];
+    HlArgs &a = P.a;
+    *launches = 0;
+    if (P.mode == 0) {
+        a.scratch = (double *)scratch;
+        a.q_begin = 0; a.q_end = c.nq;
+        fn<<<P.grid, 32 * P.warps, P.smem, st>>>(a);
+        ++*launches;
+    } else {
+        // record layout in the workspace: [bra records][ket records][bra headers][ket headers]; padding stays zero
+        cudaError_t e = cudaMemsetAsync(scratch, 0, P.scratch_bytes, st);
+        if (e != cudaSuccess) return e;
+        const long long nrb = P.mode == 1 ? c.bra.npairs : P.chunk, nrk = P.mode == 1 ? c.ket.npairs : P.chunk;
+        double *recb = (double *)scratch, *reck = recb + nrb * P.recb;
+        double *hdrb = reck + nrk * P.reck, *hdrk = hdrb + nrb * 4 * a.Kbra;
+        a.rec_b = recb; a.rec_k = reck; a.hdr_b = hdrb; a.hdr_k = hdrk;
+        P.pb.rec = recb; P.pb.hdr = hdrb; P.pk.rec = reck; P.pk.hdr = hdrk;
+        HlPairFn pfn = hl_pair_table()[P.NW];
+        for (long long q0 = 0; q0 < c.nq; q0 += P.chunk) {
+            const long long q1 = std::min(c.nq, q0 + P.chunk);
+            if (P.mode == 2 || q0 == 0) {
+                P.pb.nrec = P.mode == 1 ? nrb : q1 - q0; P.pk.nrec = P.mode == 1 ? nrk : q1 - q0;
+                P.pb.q_begin = P.pk.q_begin = q0;
+                const unsigned gb = (unsigned)std::min<long long>(P.pb.nrec, (long long)nsm * 4);
+                const unsigned gk = (unsigned)std::min<long long>(P.pk.nrec, (long long)nsm * 4);
+                if (gb) { pfn<<<gb, 128, P.pair_smem_b, st>>>(P.pb); ++*launches; }
+                if (gk) { pfn<<<gk, 128, P.pair_smem_k, st>>>(P.pk); ++*launches; }
+            }
+            a.q_begin = q0; a.q_end = q1;
+            const unsigned grid = (unsigned)std::min<long long>(q1 - q0, (long long)P.grid);
+            fn<<<grid, 32 * P.warps, P.smem, st>>>(a);
+            ++*launches;
+        }
+    }
     if (info) {
         info[0] = P.MW; info[1] = P.NW; info[2] = P.warps; info[3] = (int)P.smem; info[4] = P.ctas; info[5] = P.npass;
-        info[6] = P.a.ntile; info[7] = (int)P.grid;
+        info[6] = P.mode; info[7] = (int)P.grid;
     }
     return cudaGetLastError();
 }

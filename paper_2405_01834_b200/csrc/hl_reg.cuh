@@ -5,6 +5,8 @@
 namespace mdb {
 
 typedef void (*HlFn)(HlArgs);
+typedef void (*HlPairFn)(HlPairArgs);
+HlPairFn *hl_pair_table();            // [NW]
 HlFn *hl_table();                     // [warps == 8][MW 0..4][NW 0..4]
 
 template <int MW, int NW, int NWARPS>

@@ -317,13 +317,17 @@ int run(const PairView &b, const PairView &k, long long nq, const int32_t *qidx,
         out_strides(layout, qidx != nullptr, b.npairs, k.npairs, s.nab, s.ncd, c.s_q, c.s_bi, c.s_ki, c.s_ab, c.s_cd);
         c.boys_tab = S.boys_tab; c.rlut = fused_rlut();
         size_t need = 0;
-        const bool small = s.la + s.lb + s.lc + s.ld <= MD_WARP_LMAX && s.nhb * s.ncd <= MD_WARP_HALF;   // the warp kernel's classes
-        if ((S.variant == MD_VARIANT_HL || !small) && hl_plan(c, S.nsm, &need)) {
+        // By measurement (profiles/r02_hl_tune.md): the one-launch kernel wins from (gg|gg) upward (N~_bra N~_ket >= 16,000:
+        // (gg|gg) 27,225, (fg|hi) 43,680); below that ((ff|ff) 7,056, (ff|i) 7,056) its per-quartet phases are too short
+        // to fill a CTA and pair setup + the runtime-l kernels are faster.
+        const bool large = (long long)s.nhb * s.nhk >= 16000;
+        if ((S.variant == MD_VARIANT_HL || large) && hl_plan(c, S.nsm, &need)) {
             void *ws = nullptr;
             int e = sc.get(need, &ws);
             if (e) return e;
-            CK(hl_launch(c, S.nsm, ws, st, S.last_hl_info));
-            S.last_launches++;
+            int nl = 0;
+            CK(hl_launch(c, S.nsm, ws, st, S.last_hl_info, &nl));
+            S.last_launches += nl;
             S.last_variant = MD_VARIANT_HL;
             return MD_OK;
         }
