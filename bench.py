@@ -118,12 +118,25 @@ def cpu_baseline(K, pure, nsample):
 
 
 def ncu_traffic(variant):
-    """dram__bytes_read.sum + dram__bytes_write.sum per launch of the timed kernel, from the committed
-    ncu --set full capture of this workload (profiles/traffic.json), or None if there is none."""
+    """dram__bytes_read.sum + dram__bytes_write.sum per launch of the timed kernel from the committed ncu --set full capture
+    of this workload (profiles/traffic.json: {variant: {"bytes": B, "kernel_sources_sha": S}}), or None when the capture
+    is older than the kernel sources it describes (the sha is over csrc/fused2*.cuh|cu)."""
     try:
-        return json.load(open(os.path.join(ROOT, "profiles", "traffic.json"))).get(variant)
+        t = json.load(open(os.path.join(ROOT, "profiles", "traffic.json"))).get(variant)
     except (OSError, ValueError):
         return None
+    if not isinstance(t, dict):
+        return None
+    return t["bytes"] if t.get("kernel_sources_sha") == kernel_sources_sha(variant) else None
+
+
+def kernel_sources_sha(variant):
+    import glob
+    import hashlib
+    h = hashlib.sha1()
+    for f in sorted(glob.glob(os.path.join(ROOT, "paper_2405_01834_b200", "csrc", f"{variant}*"))):
+        h.update(open(f, "rb").read())
+    return h.hexdigest()[:16]
 
 
 def run_reference(args):
@@ -156,8 +169,98 @@ def measure_variant(dw, w, K, pure, steps, warmup, flush, barrier):
     flops = W.flops_model(2, 2, 2, 2, K * K, K * K, pure)
     return {"K": K, "pure": pure, "ms_per_step": ms / steps, "quartets_per_s": w.nquartets * steps / (ms * 1e-3),
             "model_flop_per_quartet": flops, "model_tflops": flops * w.nquartets * steps / (ms * 1e-3) / 1e12,
-            "variant": {1: "generic", 2: "fused", 3: "mma", 4: "fused2", 5: "warp"}.get(engine.md_last_variant(), "?"),
+            "variant": VARIANT_NAME.get(engine.md_last_variant(), "?"),
             "launches_per_step": engine.md_last_launch_count(), "out_bytes": out.numel() * 8}
+
+
+
+VARIANT_NAME = {1: "generic", 2: "fused", 3: "mma", 4: "fused2", 5: "warp", 6: "hl"}
+
+
+def per_class_cases():
+    """Rows of the per-class table the metric asks for ("per (la lb|lc ld) class and K"): BASELINE configs[0..3] at their
+    stated sizes.  (name, workload maker, solid output?)."""
+    from paper_2405_01834_b200 import workloads as W
+    c = [("cfg0 (pp|pp) K=1 cart n=2000", lambda: W.config1(2000), False)]
+    for K in (1, 3):
+        for pure in (True, False):
+            c.append((f"cfg1 (dd|dd) K={K} {'solid' if pure else 'cart'} n=200000", lambda K=K: W.config2(K=K), pure))
+    for (la, lb, lX, K) in [(0, 0, 0, 1), (1, 1, 1, 1), (3, 3, 3, 4), (3, 3, 6, 4)]:
+        c.append((f"cfg2 ({la}{lb}|{lX}) K={K} solid n=1000000", lambda la=la, lb=lb, lX=lX, K=K: W.config3(la, lb, lX, K=K), True))
+    for ls in [(4, 4, 4, 4), (5, 5, 5, 5), (6, 6, 6, 6), (3, 4, 5, 6)]:
+        c.append((f"cfg3 ({ls[0]}{ls[1]}|{ls[2]}{ls[3]}) K=1 solid n=20000", lambda ls=ls: W.config4(ls), True))
+    return c
+
+
+def executed_flops():
+    """FP64 flop per quartet that the kernels EXECUTE for each per-class case: DFMA x2 + DMUL + DADD thread instructions plus
+    512 per DMMA warp instruction, counted by ncu on a reduced batch (profiles/r02_executed_flops.md names the command).
+    Counts are per quartet and independent of the batch size; they are only trusted for the kernels they were taken on."""
+    try:
+        return json.load(open(os.path.join(ROOT, "profiles", "r02_executed_flops.json")))
+    except (OSError, ValueError):
+        return {}
+
+
+def measure_case(name, make, pure, steps, warmup, flush, local, hbm, counted):
+    import torch
+    from paper_2405_01834_b200 import engine
+    w = make()
+    dw = engine.DeviceWorkload(w)
+    out = dw.alloc_out(pure)
+    probe = time_steps(lambda: dw.run(pure, out), 1, warmup, flush, lambda: None)
+    steps = int(max(steps, min(200, 600.0 / max(probe, 1e-3))))          # at least 0.6 s timed, so that the clocks are sampled
+    with ClockSampler(local) as cs:
+        ms = time_steps(lambda: dw.run(pure, out), steps, 0, flush, lambda: None) / steps
+    used, nl = engine.md_last_variant(), engine.md_last_launch_count()
+    fl = w.flops_model(pure)
+    nsh = 3 if w.three_center else 4
+    in_bytes = sum(8 * (3 + 2 * s.K) for s in (w.a, w.b, w.c) + (() if w.three_center else (w.d,)))
+    out_bytes = out.numel() * 8 // w.nquartets
+    rate = w.nquartets / (ms * 1e-3)
+    tf = fl * rate / 1e12
+    gbs = (in_bytes + out_bytes) * rate / 1e9
+    row = {"case": name, "n": w.nquartets, "variant": VARIANT_NAME.get(used, str(used)), "launches": nl, "ms": ms,
+           "quartets_per_s": rate, "bound": "hbm" if fl / (in_bytes + out_bytes) < FP64_PEAK_DERIVED_TFLOPS * 1e3 / hbm else "alu",
+           "model_flop_per_quartet": fl, "model_tflops": tf, "frac_model": tf / FP64_PEAK_DERIVED_TFLOPS,
+           "algorithmic_bytes_per_quartet": in_bytes + out_bytes, "hbm_gbs": gbs, "frac_hbm": gbs / hbm, "steps": steps, "clocks": cs.summary()}
+    ex = counted.get(name)
+    if ex and ex.get("variant") == row["variant"]:
+        row["executed_flop_per_quartet"] = ex["flop_per_quartet"]
+        row["frac_executed"] = ex["flop_per_quartet"] * rate / 1e12 / FP64_PEAK_DERIVED_TFLOPS
+    else:
+        row["executed_flop_per_quartet"] = row["frac_executed"] = None
+    del dw, out
+    torch.cuda.empty_cache()
+    return row
+
+
+def run_case(args):
+    """One pass of one per-class case on a reduced batch (for ncu instruction counts): python bench.py --case NAME --count-n N"""
+    import torch
+    from paper_2405_01834_b200 import build, engine
+    build.build()
+    torch.cuda.set_device(0)
+    engine.md_init()
+    for name, make, pure in per_class_cases():
+        if name == args.case:
+            w = make()
+            n = min(args.count_n, w.nquartets)
+            import numpy as np
+            from paper_2405_01834_b200 import workloads as W
+            ia, ib, ic, id_ = w.shell_indices(np.arange(n))
+            ww = W.Workload(w.name, w.a.take(ia), w.b.take(ib), w.c.take(ic), None if w.three_center else w.d.take(id_),
+                            None, None, np.stack([np.arange(n, dtype=np.int32)] * 2, 1))
+            dw = engine.DeviceWorkload(ww)
+            out = dw.alloc_out(pure)
+            if args.variant:               # the variant AUTO picks at the case's full size, when the reduced batch would pick another
+                engine.md_set_variant({v: k for k, v in VARIANT_NAME.items()}[args.variant])
+            dw.run(pure, out)
+            torch.cuda.synchronize()
+            print(json.dumps({"case": name, "n": n, "variant": VARIANT_NAME.get(engine.md_last_variant()),
+                              "launches": engine.md_last_launch_count()}))
+            return
+    raise SystemExit(f"unknown case {args.case!r}")
 
 
 def run_ours(args):
@@ -180,7 +283,16 @@ def run_ours(args):
     flush = torch.empty(256 << 20, dtype=torch.uint8, device="cuda")
 
     K, pure = 3, True
-    w = workload(K, rank)
+    if world > 1:
+        # weak scaling: ONE seeded list of world x 200,000 quartets, rank r takes its contiguous shard (no data-path collective)
+        wall = workload(K, 0, n=NQ * world)
+        lo, hi = sharding.shard_range(wall.nquartets, rank, world)
+        ia, ib, ic, id_ = wall.shell_indices(np.arange(lo, hi))
+        w = W.Workload(wall.name, wall.a.take(ia), wall.b.take(ib), wall.c.take(ic), wall.d.take(id_), None, None,
+                       np.stack([np.arange(hi - lo, dtype=np.int32)] * 2, 1))
+        del wall
+    else:
+        w = workload(K, rank)
     dw = engine.DeviceWorkload(w)
     with ClockSampler(local) as cs:
         head = measure_variant(dw, w, K, pure, args.steps, args.warmup, flush, barrier)
@@ -237,6 +349,8 @@ def run_ours(args):
         achieved = head["model_tflops"]
         line["roofline"] = {"bound": "alu", "achieved": achieved, "peak": FP64_PEAK_DERIVED_TFLOPS, "unit": "TFLOP/s",
                             "frac": achieved / FP64_PEAK_DERIVED_TFLOPS, "traffic": ncu_traffic(head["variant"]),
+                            "frac_is": "Table-I MODEL flops (dense solid-harmonic contraction) over the peak; frac_executed counts what the kernel issues",
+                            "frac_executed": None,
                             "peak_source": "derived: 148 SM x 64 DFMA/clk x 2 x 1.965 GHz (DESIGN.md)",
                             "peak_measured_dfma_loop": dfma_tf, "peak_measured_dmma_m8n8k4_loop": dmma_tf,
                             "frac_of_measured_dfma": achieved / dfma_tf if dfma_tf else None,
@@ -251,6 +365,16 @@ def run_ours(args):
         if world == 1:
             cb, _ = cpu_baseline(K, pure, args.cpu_sample)
             line["cpu_baseline"] = cb
+            if not args.no_per_class:
+                hbm = line["roofline"]["hbm_peak_gbs_measured"] or 6550.0
+                counted = executed_flops()
+                line["per_class"] = [measure_case(nm, mk, pu, 2, 3, flush, local, hbm, counted) for nm, mk, pu in per_class_cases()]
+                head_ex = counted.get("cfg1 (dd|dd) K=3 solid n=200000")
+                if head_ex and head_ex.get("variant") == head["variant"]:
+                    ex_tf = head_ex["flop_per_quartet"] * value / 1e12
+                    line["roofline"]["executed_flop_per_quartet"] = head_ex["flop_per_quartet"]
+                    line["roofline"]["achieved_executed"] = ex_tf
+                    line["roofline"]["frac_executed"] = ex_tf / FP64_PEAK_DERIVED_TFLOPS
             if args.variants:
                 extra = []
                 for k2, p2 in ((1, True), (1, False), (3, False)):
@@ -372,7 +496,7 @@ def run_config5(args):
     Q = {pt: schwarz_factors(engine, W, mol, pt[0], pt[1], pairs[pt]) for pt in ptypes}
     torch.cuda.synchronize()
     t_schwarz = time.perf_counter() - t0
-    vname = {1: "generic", 2: "fused", 3: "mma", 4: "fused2", 5: "warp"}
+    vname = VARIANT_NAME
     rows = ["class,Kbra,Kket,pairs_bra,pairs_ket,quartets_passing,sampled,variant,ms,quartets_per_s,model_tflops,"
             "extrapolated_s"]
     rng = np.random.default_rng(5)
@@ -434,8 +558,8 @@ def run_sweep(args):
     engine.md_init()
     flush = torch.empty(256 << 20, dtype=torch.uint8, device="cuda")
     vid = {"auto": engine.VARIANT_AUTO, "generic": engine.VARIANT_GENERIC, "fused": engine.VARIANT_FUSED,
-           "mma": engine.VARIANT_MMA, "fused2": engine.VARIANT_FUSED2, "warp": engine.VARIANT_WARP}
-    vname = {1: "generic", 2: "fused", 3: "mma", 4: "fused2", 5: "warp"}
+           "mma": engine.VARIANT_MMA, "fused2": engine.VARIANT_FUSED2, "warp": engine.VARIANT_WARP, "hl": engine.VARIANT_HL}
+    vname = VARIANT_NAME
     try:
         hbm = json.load(open(os.path.join(ROOT, "MEASURED_PEAKS.json"))).get("hbm_gbs", 6550.0)
     except (OSError, ValueError):
@@ -443,7 +567,7 @@ def run_sweep(args):
     os.makedirs(os.path.join(ROOT, "gpurun_out"), exist_ok=True)
     path = os.path.join(ROOT, "gpurun_out", f"sweep_{args.sweep}.csv")
     rows = ["case,n,variant_asked,variant_used,launches,ms,quartets_per_s,model_flop_per_quartet,model_tflops,"
-            "frac_fp64_peak,out_gbs,frac_hbm"]
+            "frac_fp64_peak,out_gbs,frac_hbm,sm_mhz,throttle_reasons"]
     for label, make, pure, variants in sweep_cases(args.sweep):
         w = make()
         for v in variants:
@@ -466,13 +590,15 @@ def run_sweep(args):
                                         None if w.three_center else w.d.take(id_), None, None,
                                         np.stack([np.arange(cap, dtype=np.int32)] * 2, 1))
                 dw = engine.DeviceWorkload(ww); out = dw.alloc_out(pure)
-                ms = time_steps(lambda: dw.run(pure, out), args.steps, args.warmup, flush, lambda: None) / args.steps
+                with ClockSampler(0) as cs:
+                    ms = time_steps(lambda: dw.run(pure, out), args.steps, args.warmup, flush, lambda: None) / args.steps
+                ck = cs.summary()
                 used, nl = engine.md_last_variant(), engine.md_last_launch_count()
                 fl = ww.flops_model(pure)
                 tf = fl * ww.nquartets / (ms * 1e-3) / 1e12
                 gbs = out.numel() * 8 / (ms * 1e-3) / 1e9
                 rows.append(f"{label},{ww.nquartets},{v},{vname.get(used, used)},{nl},{ms:.4f},{ww.nquartets / (ms * 1e-3):.4e},"
-                            f"{fl},{tf:.3f},{tf / FP64_PEAK_DERIVED_TFLOPS:.4f},{gbs:.1f},{gbs / hbm:.4f}")
+                            f"{fl},{tf:.3f},{tf / FP64_PEAK_DERIVED_TFLOPS:.4f},{gbs:.1f},{gbs / hbm:.4f},{ck['sm_mhz']},{'+'.join(ck['reasons']) or 'none'}")
                 print(rows[-1], flush=True)
                 del dw, out
             finally:
@@ -489,10 +615,22 @@ def main():
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--variants", action="store_true", help="also time K=1 and Cartesian output")
     ap.add_argument("--cpu-sample", type=int, default=8000)
+    ap.add_argument("--no-per-class", action="store_true", help="headline only (skip the per-class table)")
+    ap.add_argument("--case", default=None, help="run ONE per-class case once on --count-n quartets (for ncu instruction counts)")
+    ap.add_argument("--count-n", type=int, default=2000)
+    ap.add_argument("--variant", default=None, help="with --case: force this kernel variant (generic|fused|mma|fused2|warp|hl)")
     ap.add_argument("--sweep", default=None, help="per-class table instead of the headline: l2 | configs | config5 | all | paper")
     args = ap.parse_args()
     args.warmup = max(args.warmup, 3) if args.impl == "ours" else args.warmup
-    if args.sweep:
+    if args.gpus > 1 and "WORLD_SIZE" not in os.environ and not args.sweep and not args.case:
+        # started without a launcher: re-execute under torchrun, one rank per GPU (NCCL's INFO log stays on for rank 0)
+        env = dict(os.environ, NCCL_DEBUG=os.environ.get("NCCL_DEBUG", "INFO"))
+        cmd = [sys.executable, "-m", "torch.distributed.run", "--nnodes=1", f"--nproc-per-node={args.gpus}",
+               "--master-addr", "127.0.0.1", "--master-port", os.environ.get("MASTER_PORT", "29511"), os.path.abspath(__file__)] + sys.argv[1:]
+        raise SystemExit(subprocess.call(cmd, env=env))
+    if args.case:
+        run_case(args)
+    elif args.sweep:
         run_sweep(args)
     elif args.impl == "reference":
         run_reference(args)

@@ -34,7 +34,8 @@ struct HlArgs {
     int la, lb, lc, ld;                  // ld = 0 for a one-centre ket
     int Ka, Kb, Kc, Kd, Kbra, Kket;
     int Lb, Lk, nab, ncd, nhb, nhk;
-    int mrows, mrows_pad;                // stacked rows (kb, p~) of [p~|cd]; padded to a multiple of kc2
+    int kbb, nblk;                       // bra primitives per row block of [p~|cd] (what fits shared memory); blocks
+    int mrows, mrows_pad;                // stacked rows (kb, p~) of one row block (kbb*nhb); padded to a multiple of kc2
     int kc2;                             // stacked bra rows per ring chunk of GEMM2: 8 or 16
     int nhk_pad;                         // ket Hermite rows padded to MD_HL_KC1
     int sb;                              // row stride of Hb in the scratch: >= 8*ceil(nab/8), = 4 mod 16
@@ -304,11 +305,13 @@ __device__ __forceinline__ void hl_gemm1_step(double (&acc)[MW][NW][2], const do
 
 // ---- S1 for one side of one quartet (or one shell pair): every primitive pair's Hermite tables (three warps, one
 // per axis), {p, P} header and dense H record.  ws = shared scratch of cap doubles.  rec: bra [K][nh][sb], ket
-// [cd tile][K][nh_pad][NT+4] (tile_stride = K nh_pad (NT+4)).  Ends with a barrier.
+// [cd tile][K][nh_pad][NT+4] (tile_stride = K nh_pad (NT+4)); bra primitives are grouped kbb to a row block of blk_rows
+// rows.  Ends with a barrier.
 template <int NTHR, int NT>
 __device__ __forceinline__ void hl_side(const PairView &pv, bool ket, int l1, int l2, int K1, int K2, int pure, long long ip,
                                         double *hdr, double *ws, int cap, const uint32_t *s_herm, const double *CaT,
-                                        const double *CbT, double *rec, int nh, int nh_pad, int sb, long long tile_stride) {
+                                        const double *CbT, double *rec, int nh, int nh_pad, int sb, long long tile_stride,
+                                        int kbb, int blk_rows) {
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
     long long i1 = ip, i2 = ip;
     if (pv.idx) { i1 = pv.idx[2 * ip]; i2 = pv.idx[2 * ip + 1]; }
@@ -347,7 +350,7 @@ __device__ __forceinline__ void hl_side(const PairView &pv, bool ket, int l1, in
             HlKetDst<NT> dst{rec + (long long)kp * nh_pad * (NT + 4), tile_stride};
             hl_build_H<NTHR>(l1, l2, pure, true, coef, E, T1, t1cap, s_herm, CaT, CbT, dst);
         } else {
-            HlBraDst dst{rec + (long long)kp * nh * sb, sb};
+            HlBraDst dst{rec + ((long long)(kp / kbb) * blk_rows + (long long)(kp % kbb) * nh) * sb, sb};   // row block, then primitive
             hl_build_H<NTHR>(l1, l2, pure, false, coef, E, T1, t1cap, s_herm, CaT, CbT, dst);
         }
     }
@@ -374,7 +377,7 @@ __device__ __forceinline__ void hl_stage_tables(uint32_t *s_herm, int nhm, doubl
 struct HlPairArgs {
     PairView pv;
     int ket, l1, l2, K1, K2, pure;
-    int nh, nh_pad, sb;
+    int nh, nh_pad, sb, kbb, blk_rows;
     long long tile_stride;
     long long nrec, rec_stride;
     double *rec, *hdr;                   // [nrec][rec_stride], [nrec][K1*K2][4]
@@ -402,15 +405,15 @@ __global__ void __launch_bounds__(128, 4) hl_pair_kernel(HlPairArgs g) {
         }
         hl_side<NTHR, NT>(g.pv, g.ket != 0, g.l1, g.l2, g.K1, g.K2, g.pure, ip, g.hdr + r * 4 * g.K1 * g.K2, sm + g.o_ws,
                           g.ws_doubles, s_herm, CT, CT + 28 * MD_HL_CSTR, g.rec + r * g.rec_stride, g.nh, g.nh_pad, g.sb,
-                          g.tile_stride);
+                          g.tile_stride, g.kbb, g.blk_rows);
     }
 }
 
 // Order in which one quartet's H chunks pass through the ring: for every cd tile, for every row pass of GEMM1 the
-// chunks (kk, c) of Hk, then the chunks of Hb for GEMM2.  Only the producer thread advances it.
+// chunks (kk, c) of Hk, then the chunks of Hb for GEMM2; with several bra-primitive row blocks, that per block.  Only the producer thread advances it.
 struct HlStream {
-    int j, pass, kk, c, c2;
-    __device__ __forceinline__ void reset(int c_first) { j = 0; pass = 0; kk = 0; c = c_first; c2 = -1; }
+    int j, blk, pass, kk, c, c2;
+    __device__ __forceinline__ void reset(int c_first) { j = 0; blk = 0; pass = 0; kk = 0; c = c_first; c2 = -1; }
 };
 
 template <int MW, int NW, int NWARPS>
@@ -443,7 +446,7 @@ __global__ void __launch_bounds__(32 * NWARPS, (NWARPS == 4 ? 3 : 1)) hl_kernel(
     {
         const int ls[4] = {g.la, g.lb, g.lc, g.ld};
         hl_stage_tables<NTHR>(s_herm, nherm(max(g.Lb, g.Lk)), CT, ls);
-        for (int r = tid; r < g.mrows_pad; r += NTHR) {
+        for (int r = tid; r < g.mrows_pad; r += NTHR) {            // one row block: .y = bra primitive inside the block
             const int rr = min(r, g.mrows - 1), kb = rr / nhb;
             rowinfo[r] = make_int2((int)c_herm[rr - kb * nhb], kb);
         }
@@ -456,7 +459,7 @@ __global__ void __launch_bounds__(32 * NWARPS, (NWARPS == 4 ? 3 : 1)) hl_kernel(
     long long gcons = 0, gprod = 0;                        // chunks consumed (all threads) / issued (thread 0), CTA lifetime
     HlStream ps;
     long long left = 0;                                    // chunks of the current quartet not yet issued (thread 0)
-    const long long per_quartet = (long long)g.ntile * ((long long)npass * g.Kket * (nc1 - c_first) + nc2);
+    const long long per_quartet = (long long)g.ntile * g.nblk * ((long long)npass * g.Kket * (nc1 - c_first) + nc2);
 
     auto produce = [&]() {                                 // thread 0: issue the next chunk of the stream
         const int s = (int)(gprod % ST);
@@ -468,9 +471,9 @@ __global__ void __launch_bounds__(32 * NWARPS, (NWARPS == 4 ? 3 : 1)) hl_kernel(
             bytes = bytes1;
             if (++ps.c == nc1) { ps.c = c_first; if (++ps.kk == g.Kket) { ps.kk = 0; if (++ps.pass == npass) { ps.pass = 0; ps.c2 = 0; } } }
         } else {
-            src = hb + (long long)ps.c2 * g.kc2 * g.sb;
+            src = hb + ((long long)ps.blk * g.mrows_pad + (long long)ps.c2 * g.kc2) * g.sb;
             bytes = bytes2;
-            if (++ps.c2 == nc2) { ps.c2 = -1; ++ps.j; }
+            if (++ps.c2 == nc2) { ps.c2 = -1; if (++ps.blk == g.nblk) { ps.blk = 0; ++ps.j; } }
         }
         hl_bar_expect(full + s, bytes);
         hl_bulk_g2s(ring + (size_t)s * g.ring_stage, src, bytes, full + s);
@@ -499,9 +502,9 @@ __global__ void __launch_bounds__(32 * NWARPS, (NWARPS == 4 ? 3 : 1)) hl_kernel(
         if (g.fused) {
             const int cap = g.ov_doubles + ST * g.ring_stage;
             hl_side<NTHR, NT>(g.bra, false, g.la, g.lb, g.Ka, g.Kb, g.pure, bi, hdr, ov, cap, s_herm, CT, CT + CTS, scr,
-                              nhb, 0, g.sb, 0);
+                              nhb, 0, g.sb, 0, g.kbb, g.mrows_pad);
             hl_side<NTHR, NT>(g.ket, true, g.lc, g.ld, g.Kc, g.Kd, g.pure, ki, hdr + 4 * g.Kbra, ov, cap, s_herm, CT + 2 * CTS,
-                              CT + 3 * CTS, scr + g.off_hk, nhk, g.nhk_pad, 0, hk_tile);
+                              CT + 3 * CTS, scr + g.off_hk, nhk, g.nhk_pad, 0, hk_tile, 1, 0);
         } else {
             const long long rb = g.by_quartet ? q - g.q_begin : bi, rk = g.by_quartet ? q - g.q_begin : ki;
             hb = g.rec_b + rb * g.rec_stride_b;
@@ -560,7 +563,13 @@ __global__ void __launch_bounds__(32 * NWARPS, (NWARPS == 4 ? 3 : 1)) hl_kernel(
         for (int j = 0; j < g.ntile; ++j) {
             const int cd0 = j * NT;
             const int nnt = min(NW, (g.ncd - cd0 + 7) >> 3);
-            // GEMM1 (Eqs. 19, 25): rows = stacked (kb, p~), columns = this cd tile, K = (kk, q~)
+            double c2[MD_HL_MT2][NW][2];                       // the [ab|cd] tile, summed over the row blocks
+#pragma unroll
+            for (int t = 0; t < MD_HL_MT2; ++t)
+#pragma unroll
+                for (int n = 0; n < NW; ++n) c2[t][n][0] = c2[t][n][1] = 0.0;
+            for (int blk = 0; blk < g.nblk; ++blk) {
+            // GEMM1 (Eqs. 19, 25): rows = stacked (kb, p~) of the row block, columns = this cd tile, K = (kk, q~)
             for (int pass = 0; pass < npass; ++pass) {
                 uint32_t wrow[MW];
                 int rbase[MW];
@@ -568,7 +577,7 @@ __global__ void __launch_bounds__(32 * NWARPS, (NWARPS == 4 ? 3 : 1)) hl_kernel(
                 for (int i = 0; i < MW; ++i) {                 // row tiles past the end compute on a clamped row; not stored
                     const int mt = (pass * MW + i) * NWARPS + warp;
                     const int2 ri = rowinfo[min(mt, nmt - 1) * 8 + lr];
-                    wrow[i] = (uint32_t)ri.x; rbase[i] = ri.y * g.rs0;
+                    wrow[i] = (uint32_t)ri.x; rbase[i] = min(blk * g.kbb + ri.y, g.Kbra - 1) * g.rs0;
                 }
                 double acc[MW][NW][2];
 #pragma unroll
@@ -613,11 +622,6 @@ __global__ void __launch_bounds__(32 * NWARPS, (NWARPS == 4 ? 3 : 1)) hl_kernel(
             }
             __syncthreads();
             // GEMM2 (Eq. 26): rows = ab (MD_HL_MT2 tiles per warp), columns = the cd tile, K = stacked (kb, p~)
-            double c2[MD_HL_MT2][NW][2];
-#pragma unroll
-            for (int t = 0; t < MD_HL_MT2; ++t)
-#pragma unroll
-                for (int n = 0; n < NW; ++n) c2[t][n][0] = c2[t][n][1] = 0.0;
             // specialised on the number of ab row tiles this warp owns (TC) and on a full cd tile: no guards inside
             auto gemm2 = [&](auto tc, auto full) {
                 constexpr int TC = decltype(tc)::value;
@@ -658,6 +662,8 @@ __global__ void __launch_bounds__(32 * NWARPS, (NWARPS == 4 ? 3 : 1)) hl_kernel(
                     else if (tc == 1) gemm2(integral_constant<int, 1>{}, F{});
                     else gemm2(integral_constant<int, 0>{}, F{});
                 }
+            }
+            if (blk + 1 < g.nblk) __syncthreads();             // [p~|cd] is rewritten by the next row block
             }
             // S5: the accumulators are the final [ab|cd] tile
 #pragma unroll

@@ -49,9 +49,9 @@ bool make_plan(const HlCall &c, int nsm, HlPlan &P) {
     a.Lb = a.la + a.lb; a.Lk = a.lc + a.ld;
     a.nab = ncomp(a.la, c.pure) * ncomp(a.lb, c.pure); a.ncd = ncomp(a.lc, c.pure) * ncomp(a.ld, c.pure);
     a.nhb = nherm(a.Lb); a.nhk = nherm(a.Lk);
-    a.mrows = a.Kbra * a.nhb;
     a.nhk_pad = (a.nhk + MD_HL_KC1 - 1) / MD_HL_KC1 * MD_HL_KC1;
-    const int nmt2 = (a.nab + 7) / 8, nmt = (a.mrows + 7) / 8;
+    const int nmt2 = (a.nab + 7) / 8;
+    int nmt = (a.Kbra * a.nhb + 7) / 8;                   // row tiles if all bra primitives share one row block (refined below)
     a.sb = (8 * nmt2 - 4 + 15) / 16 * 16 + 4;
     a.q_first = (c.ket.single && c.pure) ? nherm(a.lc - 1) / MD_HL_KC1 * MD_HL_KC1 : 0;
     a.qidx = c.qidx; a.nq = c.nq; a.nket = c.ket.npairs; a.out = c.out;
@@ -66,12 +66,13 @@ bool make_plan(const HlCall &c, int nsm, HlPlan &P) {
     int NW = (nnt_total + ntile - 1) / ntile;
     int warps, MW;
     // By measurement (profiles/r02_hl_tune.md): 4-warp CTAs (three per SM) for the small classes, else 8 warps; the row tiles
-    // per warp that give the fewest tile slots over all row passes, the larger on ties.
+    // per warp that give the fewest tile slots over all row passes, weighted towards larger tiles (fewer gathers per DMMA).
     warps = (nmt <= 12 && nmt2 <= 4 * MD_HL_MT2) ? 4 : 8;
     MW = 1;
-    for (int m = 1, best = 1 << 30; m <= (warps == 4 ? 3 : 4); ++m) {
-        const int slots = (nmt + warps * m - 1) / (warps * m) * m;
-        if (slots <= best) { best = slots; MW = m; }
+    double best = 1e30;
+    for (int m = 1; m <= (warps == 4 ? 3 : 4); ++m) {     // tile slots, weighted by the operand traffic per tensor-core step
+        const double cost = (nmt + warps * m - 1) / (warps * m) * m * (1.0 + 0.35 / m);
+        if (cost < best) { best = cost; MW = m; }
     }
     if (const char *f = getenv("MD_HL_FORCE")) {           // measurement override: "MW,NW,warps"
         int m, n, w;
@@ -89,7 +90,13 @@ bool make_plan(const HlCall &c, int nsm, HlPlan &P) {
     const int t1_b = c.pure ? t1_slice(a.la) : 0, t1_k = c.pure ? t1_slice(a.lc) : 0;
     const int s1_need = std::max(3 * esz_b + 2 + warps * t1_b, 3 * esz_k + 2 + warps * t1_k);
     bool fits = false;
-    for (int kc2 = 16; kc2 >= 8 && !fits; kc2 -= 8) {     // 16 stacked rows per GEMM2 chunk when shared memory allows
+    // bra primitives per row block: all of them if [p~|cd] fits shared memory, else as many as do; then 16 stacked rows
+    // per GEMM2 chunk when shared memory allows, else 8
+    for (int nblk = 1; nblk <= a.Kbra && !fits; ++nblk)
+    for (int kc2 = 16; kc2 >= 8 && !fits; kc2 -= 8) {
+        a.kbb = (a.Kbra + nblk - 1) / nblk;
+        a.nblk = (a.Kbra + a.kbb - 1) / a.kbb;
+        a.mrows = a.kbb * a.nhb;
         a.kc2 = kc2;
         a.mrows_pad = (a.mrows + kc2 - 1) / kc2 * kc2;
         a.ring_stage = up16(std::max(MD_HL_KC1 * NTS, kc2 * a.sb));
@@ -117,7 +124,7 @@ bool make_plan(const HlCall &c, int nsm, HlPlan &P) {
     P.npass = (a.mrows_pad / 8 + warps * MW - 1) / (warps * MW);
     if (!hl_table()[((warps == 8) * 5 + MW) * 5 + NW]) return false;
 
-    const long long hb_doubles = (long long)a.mrows_pad * a.sb;
+    const long long hb_doubles = (long long)a.nblk * a.mrows_pad * a.sb;
     const long long hk_doubles = (long long)a.ntile * a.Kket * a.nhk_pad * NTS;
     a.off_hk = (hb_doubles + 15) / 16 * 16;
     a.scratch_stride = (a.off_hk + hk_doubles + 15) / 16 * 16;
@@ -135,11 +142,8 @@ bool make_plan(const HlCall &c, int nsm, HlPlan &P) {
     const long long npb = c.bra.npairs, npk = c.ket.npairs;
     const size_t per_pair = 8 * ((size_t)npb * (P.recb + 4 * a.Kbra) + (size_t)npk * (P.reck + 4 * a.Kket));
     const size_t per_quartet = 8 * (size_t)(P.recb + P.reck + 4 * (a.Kbra + a.Kket));
-    if (mode < 0) {
-        if (per_pair <= budget && npb + npk <= 2 * c.nq) mode = 1;
-        else if (per_quartet * P.grid <= budget) mode = 2;
-        else mode = 0;
-    }
+    if (mode < 0)   // by measurement: records pay when pairs are shared (two quartets per pair or more); else S1 in the kernel
+        mode = (per_pair <= budget && npb + npk <= c.nq) ? 1 : 0;
     if (mode == 1 && per_pair > budget) mode = 2;
     if (mode == 2 && per_quartet * P.grid > budget) mode = 0;
     P.mode = mode;
@@ -158,6 +162,7 @@ bool make_plan(const HlCall &c, int nsm, HlPlan &P) {
         g.l1 = side ? a.lc : a.la; g.l2 = side ? a.ld : a.lb; g.K1 = side ? a.Kc : a.Ka; g.K2 = side ? a.Kd : a.Kb;
         g.pure = c.pure; g.nh = side ? a.nhk : a.nhb; g.nh_pad = side ? a.nhk_pad : 0; g.sb = side ? 0 : a.sb;
         g.tile_stride = side ? (long long)a.Kket * a.nhk_pad * NTS : 0;
+        g.kbb = side ? 1 : a.kbb; g.blk_rows = side ? 0 : a.mrows_pad;
         g.rec_stride = side ? P.reck : P.recb;
         g.by_quartet = mode == 2; g.qidx = c.qidx; g.nket = npk;
         const int esz = (g.l1 + 1) * (g.l2 + 1) * (g.l1 + g.l2 + 1);

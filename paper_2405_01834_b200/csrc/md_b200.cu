@@ -321,7 +321,10 @@ int run(const PairView &b, const PairView &k, long long nq, const int32_t *qidx,
         // (gg|gg) 27,225, (fg|hi) 43,680); below that ((ff|ff) 7,056, (ff|i) 7,056) its per-quartet phases are too short
         // to fill a CTA and pair setup + the runtime-l kernels are faster.
         const bool large = (long long)s.nhb * s.nhk >= 16000;
-        if ((S.variant == MD_VARIANT_HL || large) && hl_plan(c, S.nsm, &need)) {
+        // ... and whenever the per-pair records of the runtime-l chain would not fit a sane workspace (1 M independent
+        // contracted triplets of (ff|f): 527 GB): the one-launch kernel's scratch does not grow with the batch.
+        const bool huge_ws = generic_ws_bytes(b, k, pure) > ((size_t)8 << 30);
+        if ((S.variant == MD_VARIANT_HL || large || huge_ws) && hl_plan(c, S.nsm, &need)) {
             void *ws = nullptr;
             int e = sc.get(need, &ws);
             if (e) return e;
