@@ -460,20 +460,11 @@ def sweep_cases(name):
 
 
 def schwarz_factors(engine, W, mol, ta, tb, pairs):
-    """Q_ij = sqrt(max_ab |(ab|ab)|) for every pair of one pair type, with the engine in (i,i) quartet mode."""
+    """Q_ij = sqrt(max_ab |(ab|ab)|) for every pair of one pair type: md_schwarz on the device (csrc/screen.cu)."""
     import numpy as np
-    import torch
-    n = len(pairs)
-    nab = W.nsolid(ta[0]) * W.nsolid(tb[0])
-    q = np.empty(n)
-    step = max(1, (256 << 20) // (8 * nab * nab))
-    for lo in range(0, n, step):
-        hi = min(n, lo + step)
-        ii = np.arange(hi - lo, dtype=np.int32)
-        w = W.config5_class(mol, (ta, tb), (ta, tb), pairs[lo:hi], pairs[lo:hi], np.stack([ii, ii], 1))
-        out = engine.DeviceWorkload(w).run(True).view(hi - lo, nab, nab)
-        q[lo:hi] = torch.sqrt(torch.diagonal(out, dim1=1, dim2=2).abs().amax(dim=1)).cpu().numpy()
-    return q
+    w = W.config5_class(mol, (ta, tb), (ta, tb), pairs, pairs[:1], np.zeros((1, 2), np.int32))
+    dw = engine.DeviceWorkload(w)
+    return engine.md_schwarz(dw.a, dw.b, dw.bra_idx, True)          # torch CUDA tensor [npairs]
 
 
 def run_config5(args):
@@ -493,8 +484,9 @@ def run_config5(args):
     ptypes = mol.pair_types(4)
     pairs = {pt: mol.pair_list(*pt) for pt in ptypes}
     t0 = time.perf_counter()
-    Q = {pt: schwarz_factors(engine, W, mol, pt[0], pt[1], pairs[pt]) for pt in ptypes}
+    Qd = {pt: schwarz_factors(engine, W, mol, pt[0], pt[1], pairs[pt]) for pt in ptypes}
     torch.cuda.synchronize()
+    Q = {pt: q.cpu().numpy() for pt, q in Qd.items()}               # host copies only for drawing the timed samples
     t_schwarz = time.perf_counter() - t0
     vname = VARIANT_NAME
     rows = ["class,Kbra,Kket,pairs_bra,pairs_ket,quartets_passing,sampled,variant,ms,quartets_per_s,model_tflops,"
@@ -505,7 +497,7 @@ def run_config5(args):
     for ib, pb in enumerate(ptypes):
         for pk in ptypes[: ib + 1]:
             same = pb == pk
-            count = W.schwarz_count(Q[pb], Q[pk], thr, same)
+            count, _ = engine.md_quartet_list(Qd[pb], Qd[pk], thr, same=same, capacity=0)   # exact count on the device
             if count == 0:
                 continue
             # The timed call sees a random subset of at most 2048 pairs per side and a sample of the surviving quartets

@@ -125,6 +125,23 @@ int md_eri3_host(const md_pairs *bra, const md_shells *X,
                  int pure, int layout,
                  double *out, int64_t out_capacity_elems, void *cuda_stream);
 
+/*
+ * Screening, the step before the hot path ("Due to screening these index sets are not Cartesian
+ * products"; BASELINE config 5: "All shell quartets passing a Schwarz bound of 1e-12 are evaluated").
+ *
+ * md_schwarz: Q[i] = sqrt(max over the components ab of |(ab|ab)|) for every pair i of the batch, from the diagonal
+ *   integrals of md_eri4 in (i,i) quartet mode (pure selects the component set the maximum runs over).  Q is a DEVICE
+ *   array of npairs doubles.  Asynchronous on cuda_stream.
+ * md_quartet_list: every (i,j) with Qbra[i]*Qket[j] >= thr (one FP64 multiply), in ascending (i,j) order; same != 0
+ *   keeps only j <= i (bra and ket are the same pair list: the unique quartets).  All pointers are DEVICE memory.
+ *   *count receives the number of quartets that pass (also when it exceeds capacity); idx receives the first
+ *   min(count, capacity) of them as [k][2] = (bra pair, ket pair), ready to be passed to md_eri4 as quartet_idx.
+ *   capacity = 0 with idx = NULL only counts.  Asynchronous on cuda_stream.
+ */
+int md_schwarz(const md_pairs *pairs, int pure, double *Q, void *cuda_stream);
+int md_quartet_list(const double *Qbra, int64_t nbra, const double *Qket, int64_t nket, double thr, int same,
+                    int32_t *idx, int64_t capacity, int64_t *count, void *cuda_stream);
+
 /* Number of doubles the result occupies (negative error code on bad arguments). */
 int64_t md_eri4_out_elems(int la, int lb, int lc, int ld, int pure, int64_t nquartets);
 int64_t md_eri3_out_elems(int la, int lb, int lX, int pure, int64_t ntriplets);

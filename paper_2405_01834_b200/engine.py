@@ -30,7 +30,7 @@ class md_pairs(ctypes.Structure):
 SYMBOLS = ["md_eri4", "md_eri3", "md_eri4_host", "md_eri3_host", "md_eri4_out_elems", "md_eri3_out_elems",
            "md_eri4_workspace_bytes", "md_eri3_workspace_bytes", "md_set_workspace", "md_set_variant",
            "md_last_variant", "md_last_launch_count", "md_init", "md_boys", "md_fp64_peak", "md_strerror", "md_last_cuda_error",
-           "md_version"]
+           "md_version", "md_schwarz", "md_quartet_list"]
 
 _lib = None
 
@@ -62,6 +62,9 @@ def lib():
         L.md_set_variant.argtypes = [ctypes.c_int]
         L.md_boys.argtypes = [ctypes.c_int, ctypes.c_int, ctypes.c_int64, ctypes.c_void_p, ctypes.c_void_p, ctypes.c_void_p]
         L.md_fp64_peak.argtypes = [ctypes.c_int, ctypes.c_int, _dp, _dp]
+        L.md_schwarz.argtypes = [pp, ctypes.c_int, ctypes.c_void_p, ctypes.c_void_p]
+        L.md_quartet_list.argtypes = [ctypes.c_void_p, ctypes.c_int64, ctypes.c_void_p, ctypes.c_int64, ctypes.c_double, ctypes.c_int,
+                                      ctypes.c_void_p, ctypes.c_int64, ctypes.c_void_p, ctypes.c_void_p]
         L.md_strerror.argtypes = [ctypes.c_int]
         L.md_strerror.restype = ctypes.c_char_p
         L.md_last_cuda_error.restype = ctypes.c_char_p
@@ -220,6 +223,31 @@ def md_eri3_host(a, b, x, bra_idx, triplet_idx, ntriplets, pure, out, layout=LAY
     _check(lib().md_eri3_host(ctypes.byref(bra), ctypes.byref(xs), int(ntriplets), _ptr(triplet_idx), int(pure),
                               int(layout), _ptr(out), nout, _stream_ptr(stream)))
     return out
+
+
+def md_schwarz(a, b, pair_idx, pure, npairs=None, stream=None):
+    """Schwarz factors Q[npairs] (torch CUDA float64) of a pair batch on DEVICE tensors."""
+    import torch
+    pairs = _pairs_struct(a, b, pair_idx, npairs)
+    Q = torch.empty(pairs.npairs, dtype=torch.float64, device=a.center.device)
+    _check(lib().md_schwarz(ctypes.byref(pairs), int(pure), _ptr(Q), _stream_ptr(stream)))
+    return Q
+
+
+def md_quartet_list(Qbra, Qket, thr, same=False, capacity=None, stream=None):
+    """(count, idx[min(count, capacity), 2] int32 CUDA tensor) of the quartets with Qbra[i] Qket[j] >= thr, ascending (i, j).
+    capacity=None counts first and allocates exactly."""
+    import torch
+    count = torch.zeros(1, dtype=torch.int64, device=Qbra.device)
+    sp = _stream_ptr(stream)
+    if capacity is None:
+        _check(lib().md_quartet_list(_ptr(Qbra), Qbra.numel(), _ptr(Qket), Qket.numel(), float(thr), int(same), None, 0, _ptr(count), sp))
+        capacity = int(count.item())
+    idx = torch.empty((max(capacity, 0), 2), dtype=torch.int32, device=Qbra.device)
+    _check(lib().md_quartet_list(_ptr(Qbra), Qbra.numel(), _ptr(Qket), Qket.numel(), float(thr), int(same),
+                                 _ptr(idx) if capacity else None, capacity, _ptr(count), sp))
+    n = int(count.item())
+    return n, idx[: min(n, capacity)]
 
 
 def md_boys(mmax, T, scheme=0):
