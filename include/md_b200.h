@@ -142,6 +142,21 @@ int md_schwarz(const md_pairs *pairs, int pure, double *Q, void *cuda_stream);
 int md_quartet_list(const double *Qbra, int64_t nbra, const double *Qket, int64_t nket, double thr, int same,
                     int32_t *idx, int64_t capacity, int64_t *count, void *cuda_stream);
 
+/*
+ * Exchange digestion (Eq. 32; 389-399, Eqs. 33-35): K[b][c] += sum over the listed quartets and the
+ * components a, d of (ab|cd) D[a][d], without ever storing the integrals V[ij,ab,cd,kl] of Eq. 33.
+ *   bra / ket / quartet_idx / pure as for md_eri4 (4-center only).  off_a..off_d (DEVICE, int32): AO offset of every
+ *   shell of the four shell batches (row/column of its first component in D and K).  D and K: DEVICE [nao][nao]
+ *   row-major; K is ACCUMULATED into (zero it first); it is the caller's business which quartets it lists (Eq. 32 runs
+ *   over all a, d; permutational symmetry is not assumed).
+ * Classes with every l <= 2 are digested in the integral kernel's epilogue (one atomic per K row and thread); other
+ * classes go through an L2-sized chunk of quartet blocks and a digestion kernel.  Atomic accumulation: the summation
+ * order, hence the last bits of K, can differ from run to run.  Asynchronous on cuda_stream.
+ */
+int md_exchange(const md_pairs *bra, const md_pairs *ket, int64_t nquartets, const int32_t *quartet_idx, int pure,
+                const int32_t *off_a, const int32_t *off_b, const int32_t *off_c, const int32_t *off_d, int64_t nao,
+                const double *D, double *K, void *cuda_stream);
+
 /* Number of doubles the result occupies (negative error code on bad arguments). */
 int64_t md_eri4_out_elems(int la, int lb, int lc, int ld, int pure, int64_t nquartets);
 int64_t md_eri3_out_elems(int la, int lb, int lX, int pure, int64_t ntriplets);

@@ -1,5 +1,6 @@
 // fused_inst.cu -- instantiations of the fused kernels (canonical classes, l <= MD_FUSED_LMAX).
 #include "fused.cuh"
+#include "fused_api.cuh"
 
 namespace mdb {
 
@@ -76,7 +77,7 @@ void fused_make_args(const PairView &b0, const PairView &k0, long long nq, const
 }
 
 int fused_dispatch(const PairView &b0, const PairView &k0, long long nq, const int32_t *qidx, int pure, int layout,
-                   double *out, const double *boys_tab, int nsm, cudaStream_t st, bool /*force*/) {
+                   double *out, const double *boys_tab, int nsm, cudaStream_t st, bool /*force*/, const FusedDigest *dg) {
     if (b0.a.l > MD_FUSED_LMAX || (!b0.single && b0.b.l > MD_FUSED_LMAX) || k0.a.l > MD_FUSED_LMAX ||
         (!k0.single && k0.b.l > MD_FUSED_LMAX))
         return 0;
@@ -85,6 +86,11 @@ int fused_dispatch(const PairView &b0, const PairView &k0, long long nq, const i
     fused_make_args(b0, k0, nq, qidx, pure, layout, out, boys_tab, g, l);
     const FusedEntry &e = g_table[(((l[0] * 3 + l[1]) * 3 + l[2]) * 3 + l[3]) * 2 + (pure ? 1 : 0)];
     if (!e.fn) return 0;
+    if (dg) {                                            // kernel order: (b,a) / (d,c) when the pair was swapped
+        g.dg_K = dg->K; g.dg_D = dg->D; g.dg_n = dg->n;
+        g.dg_off[0] = dg->off[g.bra_swap ? 1 : 0]; g.dg_off[1] = dg->off[g.bra_swap ? 0 : 1];
+        g.dg_off[2] = dg->off[g.ket_swap ? 3 : 2]; g.dg_off[3] = dg->off[g.ket_swap ? 2 : 3];
+    }
     const long long ngroups = (nq + e.nq - 1) / e.nq;
     const unsigned grid = (unsigned)std::min<long long>(ngroups, (long long)nsm * e.ctas_per_sm);
     e.fn<<<grid, MD_FUSED_THREADS, e.smem, st>>>(g);

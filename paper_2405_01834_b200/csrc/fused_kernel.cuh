@@ -36,6 +36,13 @@ struct FusedArgs {
     long long sa, sb, sc, sd;     // component strides of the kernel's four shells
     const double *boys_tab;
     const uint32_t *rlut;         // [2*N~(24)]: R-recursion neighbours and packed (t,u,v)
+    // Exchange digestion (Eq. 32, K_bc += sum_ad [ab|cd] D_ad): when dg_K != nullptr nothing is stored to `out`;
+    // each thread contracts its integrals with D and adds into K.  dg_off[s] = AO offset of every shell of the kernel's
+    // shell s (kernel order, i.e. after the canonical swaps); D and K are [dg_n][dg_n], row-major.
+    double *dg_K = nullptr;
+    const double *dg_D = nullptr;
+    const int32_t *dg_off[4] = {nullptr, nullptr, nullptr, nullptr};
+    long long dg_n = 0;
 };
 
 template <int LA, int LB, int LC, int LD, bool PURE>
@@ -357,11 +364,39 @@ __global__ void __launch_bounds__(MD_FUSED_THREADS) fused_kernel(FusedArgs g) {
             long long bi, ki;
             if (g.qidx) { bi = g.qidx[2 * q]; ki = g.qidx[2 * q + 1]; }
             else { bi = q / g.nket; ki = q % g.nket; }
+            if (g.dg_K) {
+                // In caller order K[b][c] += [ab|cd] D[a][d]; the kernel's shells may be (b,a) and/or (d,c).  This thread
+                // holds one (c',d') column and all (a',b'): the D-side bra index is summed in registers, one atomic per K row.
+                long long ia = bi, ib = bi, ic = ki, id = ki;
+                if (g.bra.idx) { ia = g.bra.idx[2 * bi + g.bra_swap]; ib = g.bra.idx[2 * bi + 1 - g.bra_swap]; }
+                if (g.ket.idx) { ic = g.ket.idx[2 * ki + g.ket_swap]; id = g.ket.idx[2 * ki + 1 - g.ket_swap]; }
+                const long long oa = g.dg_off[0][ia], ob = g.dg_off[1][ib];
+                const long long oc = g.dg_off[2][ic] + icd / C::NDO, od = g.dg_off[3][id] + icd % C::NDO;
+                const long long kcol = g.ket_swap ? od : oc, dcol = g.ket_swap ? oc : od;
+                if (!g.bra_swap) {                                   // a' = a (D row), b' = b (K row)
+#pragma unroll
+                    for (int b = 0; b < C::NBO; ++b) {
+                        double s = 0.0;
+#pragma unroll
+                        for (int a = 0; a < C::NAO; ++a) s = fma(o2[a * C::NBO + b], g.dg_D[(oa + a) * g.dg_n + dcol], s);
+                        atomicAdd(g.dg_K + (ob + b) * g.dg_n + kcol, s);
+                    }
+                } else {                                             // a' = b (K row), b' = a (D row)
+#pragma unroll
+                    for (int a = 0; a < C::NAO; ++a) {
+                        double s = 0.0;
+#pragma unroll
+                        for (int b = 0; b < C::NBO; ++b) s = fma(o2[a * C::NBO + b], g.dg_D[(ob + b) * g.dg_n + dcol], s);
+                        atomicAdd(g.dg_K + (oa + a) * g.dg_n + kcol, s);
+                    }
+                }
+            } else {
             double *o = g.out + q * g.s_q + bi * g.s_bi + ki * g.s_ki + (icd / C::NDO) * g.sc + (icd % C::NDO) * g.sd;
 #pragma unroll
             for (int a = 0; a < C::NAO; ++a)
 #pragma unroll
                 for (int b = 0; b < C::NBO; ++b) o[a * g.sa + b * g.sb] = o2[a * C::NBO + b];
+            }
         }
     }
 }

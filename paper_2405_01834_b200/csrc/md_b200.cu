@@ -356,6 +356,80 @@ long long run_query(const PairView &b, const PairView &k, long long nq, int list
 }
 
 
+// ---- exchange digestion for classes without an in-kernel epilogue: [ab|cd] of a chunk of quartets goes to an L2-sized
+// scratch (never the full V of PAPER.md Eq. 33) and is contracted by this kernel (Eqs. 34-35: atomic reduction into K).
+__global__ void product_idx_kernel(int32_t *idx, long long q0, long long n, long long nket) {
+    const long long i = blockIdx.x * (long long)blockDim.x + threadIdx.x;
+    if (i < n) { idx[2 * i] = (int32_t)((q0 + i) / nket); idx[2 * i + 1] = (int32_t)((q0 + i) % nket); }
+}
+__global__ void __launch_bounds__(128) exchange_digest_kernel(const double *V, long long nq, const int32_t *qidx,
+                                                              const int32_t *bidx, const int32_t *kidx, int na, int nb, int nc,
+                                                              int nd, const int32_t *off_a, const int32_t *off_b,
+                                                              const int32_t *off_c, const int32_t *off_d, long long n,
+                                                              const double *D, double *K) {
+    for (long long q = blockIdx.x; q < nq; q += gridDim.x) {
+        const long long bi = qidx[2 * q], ki = qidx[2 * q + 1];
+        const long long ia = bidx ? bidx[2 * bi] : bi, ib = bidx ? bidx[2 * bi + 1] : bi;
+        const long long ic = kidx ? kidx[2 * ki] : ki, id = kidx ? kidx[2 * ki + 1] : ki;
+        const long long oa = off_a[ia], ob = off_b[ib], oc = off_c[ic], od = off_d[id];
+        const double *v = V + q * (long long)na * nb * nc * nd;
+        for (int t = threadIdx.x; t < nb * nc; t += blockDim.x) {
+            const int b = t / nc, c = t - b * nc;
+            double s = 0.0;
+            for (int a = 0; a < na; ++a) {
+                const double *row = v + (((long long)a * nb + b) * nc + c) * nd;
+                const double *dr = D + (oa + a) * n + od;
+                for (int d = 0; d < nd; ++d) s = fma(row[d], dr[d], s);
+            }
+            atomicAdd(K + (ob + b) * n + oc + c, s);
+        }
+    }
+}
+
+int run_exchange(const md_pairs *bra, const md_pairs *ket, long long nq, const int32_t *qidx, int pure, const int32_t *const off[4],
+                 long long nao, const double *D, double *K, cudaStream_t st) {
+    const PairView b = view(*bra), k = view(*ket);
+    if (nq == 0) return MD_OK;
+    if (!qidx && nq != b.npairs * k.npairs) return MD_EINVAL;
+    S.last_launches = 0;
+    if (fused_has_class(b, k)) {                                  // every l <= 2: digestion in the kernel epilogue, no V at all
+        FusedDigest dg{K, D, nao, {off[0], off[1], off[2], off[3]}};
+        int r = fused_dispatch(b, k, nq, qidx, pure, MD_LAYOUT_QUARTET_MAJOR, nullptr, S.boys_tab, S.nsm, st, true, &dg);
+        if (r == 1) {
+            S.last_launches++;
+            CK(cudaGetLastError());
+            S.last_variant = MD_VARIANT_FUSED;
+            return MD_OK;
+        }
+        if (r < 0) return r;
+    }
+    const int na = ncomp(b.a.l, pure), nb = ncomp(b.b.l, pure), nc = ncomp(k.a.l, pure), nd = ncomp(k.b.l, pure);
+    const long long per = (long long)na * nb * nc * nd;
+    const long long chunk = std::max<long long>(1, std::min<long long>(nq, ((long long)48 << 20) / (8 * per)));   // V chunk stays in L2
+    double *V = nullptr;
+    int32_t *ci = nullptr;
+    CK(cudaMallocAsync(&V, (size_t)chunk * per * 8, st));
+    CK(cudaMallocAsync(&ci, (size_t)chunk * 2 * sizeof(int32_t), st));
+    int e = MD_OK, launches = 0;
+    for (long long q0 = 0; q0 < nq && e == MD_OK; q0 += chunk) {
+        const long long m = std::min(chunk, nq - q0);
+        const int32_t *qi = qidx ? qidx + 2 * q0 : ci;
+        if (!qidx) { product_idx_kernel<<<(unsigned)((m + 255) / 256), 256, 0, st>>>(ci, q0, m, k.npairs); ++launches; }
+        e = run_call(b, k, m, qi, pure, MD_LAYOUT_QUARTET_MAJOR, V, m * per, st);
+        launches += S.last_launches;
+        if (e == MD_OK) {
+            exchange_digest_kernel<<<(unsigned)std::min<long long>(m, (long long)S.nsm * 16), 128, 0, st>>>(
+                V, m, qi, b.idx, k.idx, na, nb, nc, nd, off[0], off[1], off[2], off[3], nao, D, K);
+            ++launches;
+        }
+    }
+    cudaFreeAsync(ci, st);
+    cudaFreeAsync(V, st);
+    S.last_launches = launches;
+    if (e == MD_OK) CK(cudaGetLastError());
+    return e;
+}
+
 }  // namespace
 
 extern "C" {
@@ -421,6 +495,19 @@ int md_eri3(const md_pairs *bra, const md_shells *X, int64_t ntriplets, const in
     if ((e = check_shells(X))) return e;
     return run_call(view(*bra), view_single(*X), ntriplets, triplet_idx, pure, layout, out, out_capacity_elems,
                     (cudaStream_t)cuda_stream);
+}
+
+int md_exchange(const md_pairs *bra, const md_pairs *ket, int64_t nquartets, const int32_t *quartet_idx, int pure,
+                const int32_t *off_a, const int32_t *off_b, const int32_t *off_c, const int32_t *off_d, int64_t nao,
+                const double *D, double *K, void *cuda_stream) {
+    int e = check_pairs(bra);
+    if (e) return e;
+    if ((e = check_pairs(ket))) return e;
+    if ((pure != 0 && pure != 1) || nquartets < 0 || nao < 0) return MD_EINVAL;
+    if (nquartets > 0 && (!off_a || !off_b || !off_c || !off_d || !D || !K)) return MD_EINVAL;
+    if ((e = md_init())) return e;
+    const int32_t *const off[4] = {off_a, off_b, off_c, off_d};
+    return run_exchange(bra, ket, nquartets, quartet_idx, pure, off, nao, D, K, (cudaStream_t)cuda_stream);
 }
 
 int64_t md_eri4_out_elems(int la, int lb, int lc, int ld, int pure, int64_t n) {

@@ -30,7 +30,7 @@ class md_pairs(ctypes.Structure):
 SYMBOLS = ["md_eri4", "md_eri3", "md_eri4_host", "md_eri3_host", "md_eri4_out_elems", "md_eri3_out_elems",
            "md_eri4_workspace_bytes", "md_eri3_workspace_bytes", "md_set_workspace", "md_set_variant",
            "md_last_variant", "md_last_launch_count", "md_init", "md_boys", "md_fp64_peak", "md_strerror", "md_last_cuda_error",
-           "md_version", "md_schwarz", "md_quartet_list"]
+           "md_version", "md_schwarz", "md_quartet_list", "md_exchange"]
 
 _lib = None
 
@@ -65,6 +65,8 @@ def lib():
         L.md_schwarz.argtypes = [pp, ctypes.c_int, ctypes.c_void_p, ctypes.c_void_p]
         L.md_quartet_list.argtypes = [ctypes.c_void_p, ctypes.c_int64, ctypes.c_void_p, ctypes.c_int64, ctypes.c_double, ctypes.c_int,
                                       ctypes.c_void_p, ctypes.c_int64, ctypes.c_void_p, ctypes.c_void_p]
+        L.md_exchange.argtypes = [pp, pp, ctypes.c_int64, ctypes.c_void_p, ctypes.c_int] + [ctypes.c_void_p] * 4 + \
+            [ctypes.c_int64, ctypes.c_void_p, ctypes.c_void_p, ctypes.c_void_p]
         L.md_strerror.argtypes = [ctypes.c_int]
         L.md_strerror.restype = ctypes.c_char_p
         L.md_last_cuda_error.restype = ctypes.c_char_p
@@ -248,6 +250,16 @@ def md_quartet_list(Qbra, Qket, thr, same=False, capacity=None, stream=None):
                                  _ptr(idx) if capacity else None, capacity, _ptr(count), sp))
     n = int(count.item())
     return n, idx[: min(n, capacity)]
+
+
+def md_exchange(a, b, c, d, bra_idx, ket_idx, quartet_idx, nquartets, pure, offs, D, K, stream=None, nbra=None, nket=None):
+    """K[b][c] += sum_ad (ab|cd) D[a][d] over the listed quartets (Eq. 32); offs = four int32 CUDA tensors."""
+    bra = _pairs_struct(a, b, bra_idx, nbra)
+    ket = _pairs_struct(c, d, ket_idx, nket)
+    _check(lib().md_exchange(ctypes.byref(bra), ctypes.byref(ket), int(nquartets), _ptr(quartet_idx), int(pure),
+                             _ptr(offs[0]), _ptr(offs[1]), _ptr(offs[2]), _ptr(offs[3]), D.shape[0], _ptr(D), _ptr(K),
+                             _stream_ptr(stream)))
+    return K
 
 
 def md_boys(mmax, T, scheme=0):
