@@ -174,7 +174,7 @@ def measure_variant(dw, w, K, pure, steps, warmup, flush, barrier):
 
 
 
-VARIANT_NAME = {1: "generic", 2: "fused", 3: "mma", 4: "fused2", 5: "warp", 6: "hl"}
+VARIANT_NAME = {1: "generic", 2: "fused", 3: "mma", 4: "fused2", 5: "warp", 6: "hl", 7: "lowl"}
 
 
 def per_class_cases():
@@ -550,7 +550,7 @@ def run_sweep(args):
     engine.md_init()
     flush = torch.empty(256 << 20, dtype=torch.uint8, device="cuda")
     vid = {"auto": engine.VARIANT_AUTO, "generic": engine.VARIANT_GENERIC, "fused": engine.VARIANT_FUSED,
-           "mma": engine.VARIANT_MMA, "fused2": engine.VARIANT_FUSED2, "warp": engine.VARIANT_WARP, "hl": engine.VARIANT_HL}
+           "mma": engine.VARIANT_MMA, "fused2": engine.VARIANT_FUSED2, "warp": engine.VARIANT_WARP, "hl": engine.VARIANT_HL, "lowl": engine.VARIANT_LOWL}
     vname = VARIANT_NAME
     try:
         hbm = json.load(open(os.path.join(ROOT, "MEASURED_PEAKS.json"))).get("hbm_gbs", 6550.0)

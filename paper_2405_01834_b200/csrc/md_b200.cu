@@ -15,12 +15,15 @@
 #include "fused_api.cuh"
 #include "generic.cuh"
 #include "hl_api.cuh"
+#include "lowl_api.cuh"
 #include "mma_api.cuh"
 #include "pair.cuh"
 #include "warp.cuh"
 #include "peak.cuh"
 
 using namespace mdb;
+
+#define MD_LOWL_KMAX (1 << 24)   // by measurement the one-thread-per-quartet kernel wins at every contraction degree tried (K = 1..6 per shell)
 
 namespace {
 
@@ -281,6 +284,18 @@ int run(const PairView &b, const PairView &k, long long nq, const int32_t *qidx,
     const bool product_s_ket = S.variant == MD_VARIANT_AUTO && !qidx && k.a.l == 0 && (k.single || k.b.l == 0) &&
                                b.a.l + (b.single ? 0 : b.b.l) >= 4 && nq >= 8 * (b.npairs + k.npairs);
     if (product_s_ket) return run_generic(b, k, nq, qidx, pure, layout, out, st, true, sc);
+    // Every l <= 1, quartet-major output: one thread per quartet, registers only, coalesced tile stores (lowl.cuh).  By
+    // measurement (profiles/r02_lowl.md) it wins while the primitive loop is short; long contractions stay with the fused kernels.
+    if ((S.variant == MD_VARIANT_LOWL || (S.variant == MD_VARIANT_AUTO && (long long)s.Ka * s.Kb * s.Kc * s.Kd <= MD_LOWL_KMAX)) &&
+        layout == MD_LAYOUT_QUARTET_MAJOR && lowl_has_class(b, k)) {
+        if (sc.dry) { sc.need = 0; return MD_DRY; }
+        if (lowl_dispatch(b, k, nq, qidx, pure, out, S.boys_tab, S.nsm, st) == 1) {
+            S.last_launches++;
+            CK(cudaGetLastError());
+            S.last_variant = MD_VARIANT_LOWL;
+            return MD_OK;
+        }
+    }
     if (S.variant == MD_VARIANT_AUTO || S.variant == MD_VARIANT_FUSED2) {
         // By measurement (profiles/r01_sweep_l2.md): the warp-specialised kernel wins on every instantiated class
         // once the primitive loop is long enough to fill its pipeline, and on (dd|dd) for any K.
@@ -473,6 +488,7 @@ int md_init(void) {
     CK(fused2_init(S.max_smem));
     CK(mma_init(S.max_smem));
     CK(hl_init(S.max_smem, herm.data(), solid.data()));
+    CK(lowl_init(S.max_smem));
     CK(cudaDeviceSynchronize());
     S.init = true;
     S.device = dev;
@@ -535,7 +551,7 @@ int md_set_workspace(void *p, size_t bytes) {
     return MD_OK;
 }
 int md_set_variant(int v) {
-    if (v < MD_VARIANT_AUTO || v > MD_VARIANT_HL) return MD_EINVAL;
+    if (v < MD_VARIANT_AUTO || v > MD_VARIANT_LOWL) return MD_EINVAL;
     S.variant = v;
     return MD_OK;
 }
