@@ -537,7 +537,85 @@ def run_config5(args):
                       "note": "per-class rate measured on a seeded sample of the surviving quartets; counts are exact"}))
 
 
+
+def run_autotune(args):
+    """Times every candidate kernel variant on every canonical class (K = 1; K = 2 per shell for classes with all l <= 3) in the
+    independent-quartet structure and writes the measured-best table the library's AUTO consults:
+    paper_2405_01834_b200/csrc/variant_table.inc (checked in) and gpurun_out/autotune.csv (all timings)."""
+    import numpy as np
+    import torch
+    from paper_2405_01834_b200 import build, engine, workloads as W
+    build.build()
+    torch.cuda.set_device(0)
+    engine.md_init()
+    os.environ["MD_NO_TABLE"] = "1"                       # candidates are forced explicitly; AUTO below means the RULES
+    flush = torch.empty(256 << 20, dtype=torch.uint8, device="cuda")
+    vid = {"rules": 0, "generic": 1, "fused": 2, "mma": 3, "fused2": 4, "warp": 5, "hl": 6, "lowl": 7}
+    pairs = [(a, b) for a in range(7) for b in range(a + 1)]
+    cases = []
+    for ib, b in enumerate(pairs):
+        for k in pairs[: ib + 1]:
+            cases.append((b + k, False))
+    for b in pairs:
+        for lX in range(7):
+            cases.append((b + (lX,), True))
+    rows = ["class,three_center,contracted,n,variant_asked,variant_used,ms,quartets_per_s"]
+    table = []
+    with ClockSampler(0) as cs:
+        for ls, three in cases:
+            lmax = max(ls)
+            for contracted in ((False, True) if lmax <= 3 else (False,)):
+                nout = 1
+                for l in ls:
+                    nout *= 2 * l + 1
+                fl = W.flops_model(ls[0], ls[1], ls[2], 0 if three else ls[3], 4 if contracted else 1,
+                                   (2 if three else 4) if contracted else 1, True)
+                n = int(max(296, min(100_000, (1 << 28) // (8 * nout), 4e10 / fl)))
+                K = tuple((2 if contracted else 1) for _ in ls)
+                w = W.independent_quartets("at", ls, K, n, (0.3, 10.0), (-4.0, 4.0), W.class_seed("at", ls, contracted), three_center=three)
+                if lmax <= 1:
+                    cands = ["lowl", "fused", "fused2"]
+                elif lmax <= 2:
+                    cands = ["fused", "fused2"]
+                else:
+                    cands = ["warp", "mma", "hl"]
+                dw = engine.DeviceWorkload(w); out = dw.alloc_out(True)
+                best = None
+                seen = set()
+                for c in cands:
+                    engine.md_set_variant(vid[c])
+                    try:
+                        ms = time_steps(lambda: dw.run(True, out), 2, 2, flush, lambda: None) / 2
+                        used = VARIANT_NAME.get(engine.md_last_variant(), "?")
+                    except engine.MDError as e:
+                        rows.append(f"{ls},{int(three)},{int(contracted)},{n},{c},error{e.code},,")
+                        continue
+                    finally:
+                        engine.md_set_variant(0)
+                    rows.append(f"{'-'.join(map(str, ls))},{int(three)},{int(contracted)},{n},{c},{used},{ms:.4f},{n / (ms * 1e-3):.4e}")
+                    if used in seen:
+                        continue                          # the forced variant fell through to one already timed
+                    seen.add(used)
+                    if best is None or ms < best[0]:
+                        best = (ms, used)
+                if best:
+                    l4 = tuple(ls) + ((0,) if three else ())
+                    table.append((l4, three, contracted, best[1]))
+                del dw, out
+    ck = cs.summary()
+    os.makedirs(os.path.join(ROOT, "gpurun_out"), exist_ok=True)
+    open(os.path.join(ROOT, "gpurun_out", "autotune.csv"), "w").write("\n".join(rows) + "\n")
+    inc = ["// generated by `python bench.py --sweep autotune` (profiles/r02_autotune.md); {la, lb, lc, ld, three-center, contracted, variant}"]
+    for l4, three, contracted, v in table:
+        inc.append(f"    {{{l4[0]}, {l4[1]}, {l4[2]}, {l4[3]}, {int(three)}, {int(contracted)}, {vid[v]}}},   // {v}")
+    open(os.path.join(ROOT, "gpurun_out", "variant_table.inc"), "w").write("\n".join(inc) + "\n")
+    print(json.dumps({"sweep": "autotune", "classes": len(table), "timings": len(rows) - 1, "clocks": ck,
+                      "table": "gpurun_out/variant_table.inc", "csv": "gpurun_out/autotune.csv"}))
+
+
 def run_sweep(args):
+    if args.sweep == "autotune":
+        return run_autotune(args)
     if args.sweep == "config5":
         return run_config5(args)
     import numpy as np

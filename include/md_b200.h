@@ -113,6 +113,15 @@ int md_eri3(const md_pairs *bra, const md_shells *X,
             int pure, int layout,
             double *out, int64_t out_capacity_elems, void *cuda_stream);
 
+/*
+ * 2-center integrals (X|Y) (the metric of density fitting): both sides are single shells
+ * expanded about their own centres with the one-centre coefficients of PAPER.md Eqs. 6, 8, 11, 12.
+ *   pair t = (X shell pair_idx[2t], Y shell pair_idx[2t+1]); NULL = the full product, t = x*Y->n + y.
+ *   out[t][mX][mY] (MD_LAYOUT_QUARTET_MAJOR) or the paper layout with X as the "bra" index.  DEVICE pointers, asynchronous.
+ */
+int md_eri2(const md_shells *X, const md_shells *Y, int64_t npairs, const int32_t *pair_idx, int pure, int layout,
+            double *out, int64_t out_capacity_elems, void *cuda_stream);
+
 /* Host-buffer forms: every array pointer (inside the structs too) is HOST memory.  The call
  * copies inputs to the device, runs the same kernels, copies the result back into `out`
  * and synchronises `cuda_stream` before returning. */

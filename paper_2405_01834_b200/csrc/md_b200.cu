@@ -5,6 +5,7 @@
 #include <algorithm>
 #include <cmath>
 #include <cstdio>
+#include <cstdlib>
 #include <cstring>
 #include <mutex>
 #include <vector>
@@ -43,6 +44,24 @@ struct State {
     int max_smem = 227 * 1024;
     char cuda_err[256] = "";
 } S;
+
+// Measured-best variant per (canonical class, contracted or not), written by `python bench.py --sweep autotune` on one
+// B200 for the independent-quartet structure (profiles/r02_autotune.md) and checked in.  Classes that are missing, and calls the
+// table cannot describe (paper layout, huge per-pair records, the product-mode exceptions), follow the rules in run().
+struct VariantRow { signed char la, lb, lc, ld, three, contracted, variant; };
+const VariantRow g_variant_table[] = {
+#include "variant_table.inc"
+    {-1, -1, -1, -1, 0, 0, 0}};
+
+int table_variant(int la, int lb, int lc, int ld, bool three, bool contracted) {
+    if (la < lb) std::swap(la, lb);
+    if (!three && lc < ld) std::swap(lc, ld);
+    if (!three && (la < lc || (la == lc && lb < ld))) { std::swap(la, lc); std::swap(lb, ld); }   // bra >= ket (sweep 6 order)
+    for (const VariantRow *r = g_variant_table; r->la >= 0; ++r)
+        if (r->la == la && r->lb == lb && r->lc == lc && r->ld == ld && (r->three != 0) == three && (r->contracted != 0) == contracted)
+            return r->variant;
+    return 0;
+}
 
 int cuda_fail(cudaError_t e) {
     snprintf(S.cuda_err, sizeof(S.cuda_err), "%s", cudaGetErrorString(e));
@@ -265,8 +284,8 @@ int run_generic(const PairView &b, const PairView &k, long long nq, const int32_
     return MD_OK;
 }
 
-int run(const PairView &b, const PairView &k, long long nq, const int32_t *qidx, int pure, int layout,
-        double *out, long long cap, cudaStream_t st, Scratch &sc) {
+int run_rules(const PairView &b, const PairView &k, long long nq, const int32_t *qidx, int pure, int layout,
+              double *out, long long cap, cudaStream_t st, Scratch &sc) {
     if (pure != 0 && pure != 1) return MD_EINVAL;
     if (layout != MD_LAYOUT_QUARTET_MAJOR && layout != MD_LAYOUT_PAPER) return MD_EINVAL;
     if (layout == MD_LAYOUT_PAPER && qidx) return MD_EINVAL;
@@ -351,6 +370,23 @@ int run(const PairView &b, const PairView &k, long long nq, const int32_t *qidx,
         }
     }
     return run_generic(b, k, nq, qidx, pure, layout, out, st, S.variant != MD_VARIANT_GENERIC, sc);
+}
+
+// AUTO: the checked-in table first (a forced variant for this one call), then the rules.
+int run(const PairView &b, const PairView &k, long long nq, const int32_t *qidx, int pure, int layout,
+        double *out, long long cap, cudaStream_t st, Scratch &sc) {
+    if (S.variant != MD_VARIANT_AUTO || (pure != 0 && pure != 1) || getenv("MD_NO_TABLE")) return run_rules(b, k, nq, qidx, pure, layout, out, cap, st, sc);
+    const Shape s = shape_of(b, k, pure);
+    const bool product_mode = !qidx && nq > 1;
+    int tv = 0;
+    if (!product_mode && layout == MD_LAYOUT_QUARTET_MAJOR && !b.single)
+        tv = table_variant(s.la, s.lb, s.lc, s.ld, k.single != 0, (long long)s.Ka * s.Kb * s.Kc * s.Kd > 1);
+    if ((tv == MD_VARIANT_WARP || tv == MD_VARIANT_MMA || tv == MD_VARIANT_GENERIC) && generic_ws_bytes(b, k, pure) > ((size_t)8 << 30)) tv = 0;
+    if (!tv) return run_rules(b, k, nq, qidx, pure, layout, out, cap, st, sc);
+    S.variant = tv;
+    const int e = run_rules(b, k, nq, qidx, pure, layout, out, cap, st, sc);
+    S.variant = MD_VARIANT_AUTO;
+    return e;
 }
 
 int run_call(const PairView &b, const PairView &k, long long nq, const int32_t *qidx, int pure, int layout,
@@ -524,6 +560,32 @@ int md_exchange(const md_pairs *bra, const md_pairs *ket, int64_t nquartets, con
     if ((e = md_init())) return e;
     const int32_t *const off[4] = {off_a, off_b, off_c, off_d};
     return run_exchange(bra, ket, nquartets, quartet_idx, pure, off, nao, D, K, (cudaStream_t)cuda_stream);
+}
+
+int md_eri2(const md_shells *X, const md_shells *Y, int64_t npairs, const int32_t *pair_idx, int pure, int layout,
+            double *out, int64_t out_capacity_elems, void *cuda_stream) {
+    int e = check_shells(X);
+    if (e) return e;
+    if ((e = check_shells(Y))) return e;
+    if (pure != 0 && pure != 1) return MD_EINVAL;
+    if (layout != MD_LAYOUT_QUARTET_MAJOR && layout != MD_LAYOUT_PAPER) return MD_EINVAL;
+    if (layout == MD_LAYOUT_PAPER && pair_idx) return MD_EINVAL;
+    if (npairs < 0 || (!pair_idx && npairs != X->n * Y->n)) return MD_EINVAL;
+    if ((long long)ncomp(X->l, pure) * ncomp(Y->l, pure) * npairs > out_capacity_elems) return MD_ECAPACITY;
+    if (npairs > 0 && !out) return MD_EINVAL;
+    if ((e = md_init())) return e;
+    S.last_launches = 0;
+    if (npairs == 0) return MD_OK;
+    // Both sides are one-centre expansions (Eqs. 6, 8, 11, 12); the runtime-l chain is side-agnostic.
+    Scratch sc;
+    sc.st = (cudaStream_t)cuda_stream;
+    const int saved = S.variant;
+    if (S.variant == MD_VARIANT_AUTO || S.variant > MD_VARIANT_WARP || S.variant == MD_VARIANT_FUSED || S.variant == MD_VARIANT_FUSED2)
+        S.variant = MD_VARIANT_WARP;                    // warp kernel where the class is small enough, else DMMA
+    e = run_generic(view_single(*X), view_single(*Y), npairs, pair_idx, pure, layout, out, sc.st, S.variant != MD_VARIANT_GENERIC, sc);
+    S.variant = saved;
+    sc.release();
+    return e;
 }
 
 int64_t md_eri4_out_elems(int la, int lb, int lc, int ld, int pure, int64_t n) {

@@ -30,7 +30,7 @@ class md_pairs(ctypes.Structure):
 SYMBOLS = ["md_eri4", "md_eri3", "md_eri4_host", "md_eri3_host", "md_eri4_out_elems", "md_eri3_out_elems",
            "md_eri4_workspace_bytes", "md_eri3_workspace_bytes", "md_set_workspace", "md_set_variant",
            "md_last_variant", "md_last_launch_count", "md_init", "md_boys", "md_fp64_peak", "md_strerror", "md_last_cuda_error",
-           "md_version", "md_schwarz", "md_quartet_list", "md_exchange"]
+           "md_version", "md_schwarz", "md_quartet_list", "md_exchange", "md_eri2"]
 
 _lib = None
 
@@ -65,6 +65,8 @@ def lib():
         L.md_schwarz.argtypes = [pp, ctypes.c_int, ctypes.c_void_p, ctypes.c_void_p]
         L.md_quartet_list.argtypes = [ctypes.c_void_p, ctypes.c_int64, ctypes.c_void_p, ctypes.c_int64, ctypes.c_double, ctypes.c_int,
                                       ctypes.c_void_p, ctypes.c_int64, ctypes.c_void_p, ctypes.c_void_p]
+        L.md_eri2.argtypes = [ps, ps] + sig
+        L.md_eri2.restype = ctypes.c_int
         L.md_exchange.argtypes = [pp, pp, ctypes.c_int64, ctypes.c_void_p, ctypes.c_int] + [ctypes.c_void_p] * 4 + \
             [ctypes.c_int64, ctypes.c_void_p, ctypes.c_void_p, ctypes.c_void_p]
         L.md_strerror.argtypes = [ctypes.c_int]
@@ -250,6 +252,14 @@ def md_quartet_list(Qbra, Qket, thr, same=False, capacity=None, stream=None):
                                  _ptr(idx) if capacity else None, capacity, _ptr(count), sp))
     n = int(count.item())
     return n, idx[: min(n, capacity)]
+
+
+def md_eri2(x, y, pair_idx, npairs, pure, out, layout=LAYOUT_QUARTET_MAJOR, stream=None):
+    """(X|Y) on DEVICE tensors; out[t][mX][mY].  Asynchronous."""
+    xs, ys = _shells_struct(x), _shells_struct(y)
+    _check(lib().md_eri2(ctypes.byref(xs), ctypes.byref(ys), int(npairs), _ptr(pair_idx), int(pure), int(layout), _ptr(out),
+                         out.numel(), _stream_ptr(stream)))
+    return out
 
 
 def md_exchange(a, b, c, d, bra_idx, ket_idx, quartet_idx, nquartets, pure, offs, D, K, stream=None, nbra=None, nket=None):
