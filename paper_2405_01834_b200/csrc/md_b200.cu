@@ -176,17 +176,25 @@ bool fused_has_class(const PairView &b, const PairView &k) {
 }
 int scratch_get(void *ctx, size_t bytes, void **out) { return ((Scratch *)ctx)->get(bytes, out); }
 
-int launch_pair_setup(const PairView &pv, int pure, int ket_sign, long long stride, double *rec, cudaStream_t st) {
+__global__ void iota2_kernel(int32_t *idx, long long n) {
+    const long long i = blockIdx.x * (long long)blockDim.x + threadIdx.x;
+    if (i < n) { idx[2 * i] = (int32_t)i; idx[2 * i + 1] = (int32_t)i; }
+}
+
+int launch_pair_setup(const PairView &pv, int pure, int ket_sign, long long stride, double *rec, cudaStream_t st,
+                      const int32_t *by_quartet = nullptr, long long q0 = 0, long long nrec = -1) {
     const int la = pv.a.l, lb = pv.single ? 0 : pv.b.l;
     const int Kab = pv.a.K * (pv.single ? 1 : pv.b.K);
-    if (pv.npairs == 0) return MD_OK;
+    if (pv.npairs == 0 || nrec == 0) return MD_OK;
     PairSetupArgs a;
     a.pv = pv; a.pure = pure; a.ket_sign = ket_sign; a.stride = stride; a.rec = rec;
+    a.by_quartet = by_quartet; a.q0 = q0; a.side = ket_sign;
+    if (nrec >= 0) a.pv.npairs = nrec;
     const int esz = (la + 1) * (lb + 1) * (la + lb + 1);
     const int rowsz = ncart(la) * nsolid(lb);
     a.pchunk = std::max(1, std::min(nherm(la + lb), 4096 / rowsz));
     size_t smem = 8 * ((size_t)3 * esz + (pure ? (size_t)a.pchunk * rowsz : 0));
-    long long nblk = pv.npairs * Kab;
+    long long nblk = a.pv.npairs * Kab;
     if (nblk > 0x7fffffffLL) return MD_EINVAL;
     switch (std::max(la, lb)) {
         case 0: pair_setup_kernel<0><<<(unsigned)nblk, 128, smem, st>>>(a); break;
@@ -214,16 +222,54 @@ void out_strides(int layout, bool list_mode, long long nbra, long long nket, int
     }
 }
 
+int run_generic_once(const PairView &b, const PairView &k, long long nq, const int32_t *qidx, int pure, int layout,
+                     double *out, cudaStream_t st, bool use_mma, Scratch &sc, void *ws, const int32_t *by_quartet, long long q0);
+
+// Per-pair records grow with the pair batch (527 KB per (ff| pair at K = 4); a quartet LIST whose records would exceed
+// MD_GEN_WS_BYTES is cut into chunks of quartets: records per quartet side (pair setup indexed by quartet), an identity
+// index list for the quartet kernel, the same scratch reused by every chunk.
+#define MD_GEN_WS_BYTES ((size_t)4 << 30)
 int run_generic(const PairView &b, const PairView &k, long long nq, const int32_t *qidx, int pure, int layout,
                 double *out, cudaStream_t st, bool use_mma, Scratch &sc) {
+    const size_t full = generic_ws_bytes(b, k, pure);
+    if (full <= MD_GEN_WS_BYTES || !qidx || layout != MD_LAYOUT_QUARTET_MAJOR) {
+        void *ws = nullptr;
+        int e = sc.get(full, &ws);
+        if (e) return e;
+        return run_generic_once(b, k, nq, qidx, pure, layout, out, st, use_mma, sc, ws, nullptr, 0);
+    }
     Shape s = shape_of(b, k, pure);
+    const size_t per = 8 * ((size_t)s.Ka * s.Kb * s.stride_b + (size_t)s.Kc * s.Kd * s.stride_k) + 2 * sizeof(int32_t);
+    const long long chunk = std::max<long long>(1, std::min<long long>(nq, (long long)(MD_GEN_WS_BYTES / per)));
     void *ws = nullptr;
-    int e = sc.get(generic_ws_bytes(b, k, pure), &ws);
+    int e = sc.get((size_t)chunk * per, &ws);
     if (e) return e;
+    int32_t *iota = (int32_t *)((char *)ws + (size_t)chunk * (per - 2 * sizeof(int32_t)));
+    iota2_kernel<<<(unsigned)((chunk + 255) / 256), 256, 0, st>>>(iota, chunk);
+    int launches = 1;
+    PairView bc = b, kc = k;
+    bc.npairs = chunk; kc.npairs = chunk;
+    for (long long q0 = 0; q0 < nq; q0 += chunk) {
+        const long long m = std::min(chunk, nq - q0);
+        bc.npairs = m; kc.npairs = m;
+        S.last_launches = 0;
+        e = run_generic_once(bc, kc, m, iota, pure, layout, out + q0 * (long long)s.nab * s.ncd, st, use_mma, sc, ws, qidx, q0);
+        launches += S.last_launches;
+        if (e) return e;
+    }
+    S.last_launches = launches;
+    return MD_OK;
+}
+
+int run_generic_once(const PairView &b, const PairView &k, long long nq, const int32_t *qidx, int pure, int layout,
+                     double *out, cudaStream_t st, bool use_mma, Scratch &sc, void *ws, const int32_t *by_quartet, long long q0) {
+    Shape s = shape_of(b, k, pure);
+    int e;
+    (void)sc;
     double *rec_b = (double *)ws;
     double *rec_k = rec_b + (size_t)b.npairs * s.Ka * s.Kb * s.stride_b;
-    if ((e = launch_pair_setup(b, pure, 0, s.stride_b, rec_b, st))) return e;
-    if ((e = launch_pair_setup(k, pure, 1, s.stride_k, rec_k, st))) return e;
+    if ((e = launch_pair_setup(b, pure, 0, s.stride_b, rec_b, st, by_quartet, q0, by_quartet ? nq : -1))) return e;
+    if ((e = launch_pair_setup(k, pure, 1, s.stride_k, rec_k, st, by_quartet, q0, by_quartet ? nq : -1))) return e;
 
     GenericArgs g;
     g.rec_bra = rec_b; g.rec_ket = rec_k; g.stride_bra = s.stride_b; g.stride_ket = s.stride_k;
@@ -355,10 +401,7 @@ int run_rules(const PairView &b, const PairView &k, long long nq, const int32_t 
         // (gg|gg) 27,225, (fg|hi) 43,680); below that ((ff|ff) 7,056, (ff|i) 7,056) its per-quartet phases are too short
         // to fill a CTA and pair setup + the runtime-l kernels are faster.
         const bool large = (long long)s.nhb * s.nhk >= 16000;
-        // ... and whenever the per-pair records of the runtime-l chain would not fit a sane workspace (1 M independent
-        // contracted triplets of (ff|f): 527 GB): the one-launch kernel's scratch does not grow with the batch.
-        const bool huge_ws = generic_ws_bytes(b, k, pure) > ((size_t)8 << 30);
-        if ((S.variant == MD_VARIANT_HL || large || huge_ws) && hl_plan(c, S.nsm, &need)) {
+        if ((S.variant == MD_VARIANT_HL || large) && hl_plan(c, S.nsm, &need)) {
             void *ws = nullptr;
             int e = sc.get(need, &ws);
             if (e) return e;
@@ -381,11 +424,11 @@ int run(const PairView &b, const PairView &k, long long nq, const int32_t *qidx,
     int tv = 0;
     if (!product_mode && layout == MD_LAYOUT_QUARTET_MAJOR && !b.single)
         tv = table_variant(s.la, s.lb, s.lc, s.ld, k.single != 0, (long long)s.Ka * s.Kb * s.Kc * s.Kd > 1);
-    if ((tv == MD_VARIANT_WARP || tv == MD_VARIANT_MMA || tv == MD_VARIANT_GENERIC) && generic_ws_bytes(b, k, pure) > ((size_t)8 << 30)) tv = 0;
     if (!tv) return run_rules(b, k, nq, qidx, pure, layout, out, cap, st, sc);
     S.variant = tv;
-    const int e = run_rules(b, k, nq, qidx, pure, layout, out, cap, st, sc);
+    int e = run_rules(b, k, nq, qidx, pure, layout, out, cap, st, sc);
     S.variant = MD_VARIANT_AUTO;
+    if (e == MD_ENOMEM) e = run_rules(b, k, nq, qidx, pure, layout, out, cap, st, sc);   // caller buffer too small for the table's choice
     return e;
 }
 

@@ -59,6 +59,10 @@ struct PairSetupArgs {
     int pchunk;              // Hermite rows per shared-memory chunk of the solid transform
     long long stride;        // doubles per (pair, primitive) record
     double *rec;             // [npairs][Ka*Kb][stride]
+    // chunked list mode (md_b200.cu::run_generic): record r belongs to the bra (side 0) or ket (side 1) pair of quartet q0 + r
+    const int32_t *by_quartet = nullptr;
+    long long q0 = 0;
+    int side = 0;
 };
 
 // One CTA per (pair, primitive pair).  Shared memory: 3 axis tables + the stage-A buffer.
@@ -83,7 +87,8 @@ __global__ void __launch_bounds__(128) pair_setup_kernel(PairSetupArgs g) {
     for (int i = threadIdx.x; i < nsolid(lb) * ncart(lb); i += blockDim.x) s_Cb[i] = c_solid[solid_off(lb) + i];
 
     const long long rid = blockIdx.x;   // pair * Ka*Kb + prim
-    const long long ipair = rid / (Ka * Kb);
+    long long ipair = rid / (Ka * Kb);
+    if (g.by_quartet) ipair = g.by_quartet[2 * (g.q0 + ipair) + g.side];
     const int kp = (int)(rid % (Ka * Kb)), ka = kp / Kb, kb = kp % Kb;
     long long ia = ipair, ib = ipair;
     if (pv.idx) { ia = pv.idx[2 * ipair]; ib = pv.idx[2 * ipair + 1]; }

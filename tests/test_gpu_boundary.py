@@ -91,3 +91,16 @@ def test_workspace_query_scales_with_the_call_not_the_class():
     w = W.config4((6, 6, 6, 6), n=64)
     dw = engine.DeviceWorkload(w)
     assert dw.workspace_bytes(True) > 0
+
+
+def test_quartet_list_is_chunked_when_pair_records_exceed_the_scratch_budget():
+    """(ff|f) with K = 4 per bra shell: 527 KB of pair records per triplet; 9,000 independent triplets would take 4.7 GB in
+    one piece (1 M triplets: 527 GB).  The runtime-l chain cuts the list into chunks that reuse a 4 GB scratch."""
+    w = W.config3(3, 3, 3, K=4, n=9000)
+    dw = engine.DeviceWorkload(w)
+    assert dw.workspace_bytes(True) <= (4 << 30) + (1 << 20)
+    out = dw.run(True)
+    torch.cuda.synchronize()
+    assert engine.md_last_launch_count() > 3                          # several chunks: pair setup x 2 + quartet kernel each
+    sel = np.concatenate([np.arange(0, 9000, 450), [8999]])
+    assert_parity(out.cpu().numpy().reshape(9000, -1)[sel], oracle_run(w, True, sel), "chunked list")
