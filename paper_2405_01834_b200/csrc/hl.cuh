@@ -128,6 +128,8 @@ __device__ __forceinline__ void hl_e_axis_warp(int la, int lb, double za, double
 struct HlBraDst {            // [kb*nhb + p~][sb]
     double *base; int sb;
     __device__ __forceinline__ double *operator()(int p, int m) const { return base + (long long)p * sb + m; }
+    __device__ __forceinline__ long long row(int p) const { return (long long)p * sb; }
+    __device__ __forceinline__ int col(int m) const { return m; }
 };
 template <int NT>
 struct HlKetDst {            // tile-major: [cd tile][kk][q~ (padded)][NT + 4]
@@ -136,6 +138,8 @@ struct HlKetDst {            // tile-major: [cd tile][kk][q~ (padded)][NT + 4]
         const int j = m / NT, n = m - j * NT;
         return base + j * tile_stride + (long long)q * (NT + 4) + n;
     }
+    __device__ __forceinline__ long long row(int q) const { return (long long)q * (NT + 4); }
+    __device__ __forceinline__ int col(int m) const { const int j = m / NT; return (int)(j * tile_stride) + m - j * NT; }
 };
 
 // ---- S1: dense H of one primitive pair (Eqs. 7, 17), all threads of the CTA ---------------------------------
@@ -187,19 +191,35 @@ __device__ __forceinline__ void hl_build_H(int la, int lb, int pure, bool neg, d
     double *T1w = T1 + (size_t)warp * pw * nca * TS;                       // needs t1cap >= NWARPS * pw * nca * TS (host)
     (void)t1cap;
     double cbf[7][2], caf[7][2];                            // constant fragments: C^{lb}[b][mb], C^{la}[a][ma]
-    uint32_t boff[7];                                       // per K step: offsets bx*nt | by*nt << 8 | bz*nt << 16 of b = 4k + lc
+    // Lane constants of the two stages, so that the inner loops are loads and tensor-core steps only: table offsets of
+    // b = 4k + lc on the three axes (b past the shell reads entry 0: finite, and its C^{lb} row is zero), T1 row offsets of
+    // a = 4k + lc, and the scratch offsets of the eight H elements this lane owns in stage B.
+    int ox[7], oy[7], oz[7], ta[7];
 #pragma unroll
     for (int k = 0; k < 7; ++k) {
         const int b = 4 * k + lc;
         int bx = 0, by = 0, bz = 0;
         if (b < ncb) unpack_tuv(cb[b], bx, by, bz);
-        boff[k] = (uint32_t)(bx * nt) | (uint32_t)(by * nt) << 8 | (uint32_t)(bz * nt) << 16;
+        ox[k] = bx * nt; oy[k] = by * nt; oz[k] = bz * nt;
+        ta[k] = min(b, nca - 1) * TS;                          // a past the shell: any finite row, its C^{la} row is zero
 #pragma unroll
         for (int n = 0; n < 2; ++n) {
             cbf[k][n] = b < ncb ? CbT[b * MD_HL_CSTR + 8 * n + lr] : 0.0;
             caf[k][n] = b < nca ? CaT[b * MD_HL_CSTR + 8 * n + lr] : 0.0;    // same lane pattern: a = 4k + lc, ma = 8n + lr
         }
     }
+    int hoff[2][2][2];
+    bool hval[2][2][2];
+#pragma unroll
+    for (int i = 0; i < 2; ++i)
+#pragma unroll
+        for (int n = 0; n < 2; ++n)
+#pragma unroll
+            for (int e = 0; e < 2; ++e) {
+                const int ma = 8 * i + lr, mb = 8 * n + 2 * lc + e;
+                hval[i][n][e] = ma < nsa && mb < nsb;
+                hoff[i][n][e] = hval[i][n][e] ? dst.col(ma * nsb + mb) : 0;
+            }
     for (int h0 = warp * pw; h0 < nh; h0 += NWARPS * pw) {
         const int hc = min(pw, nh - h0);
         const int nrows = hc * nca, nmt = (nrows + 7) >> 3;
@@ -217,11 +237,7 @@ __device__ __forceinline__ void hl_build_H(int la, int lb, int pure, bool neg, d
             double x[7];
             uint32_t live = 0;
 #pragma unroll
-            for (int k = 0; k < 7; ++k) {
-                const uint32_t o = boff[k];
-                x[k] = ex[o & 0xff] * ey[o >> 8 & 0xff] * ez[o >> 16];
-                if (!rv || 4 * k + lc >= ncb) x[k] = 0.0;
-            }
+            for (int k = 0; k < 7; ++k) x[k] = ex[ox[k]] * ey[oy[k]] * ez[oz[k]];   // rows past the end repeat the last row: not stored
 #pragma unroll
             for (int k = 0; k < 7; ++k) live |= (__any_sync(0xffffffffu, x[k] != 0.0) ? 1u : 0u) << k;
 #pragma unroll
@@ -250,13 +266,7 @@ __device__ __forceinline__ void hl_build_H(int la, int lb, int pure, bool neg, d
             double b0[7], b1[7];
             uint32_t live = 0;
 #pragma unroll
-            for (int k = 0; k < 7; ++k) {
-                const int a = min(4 * k + lc, nca - 1);
-                b0[k] = t1[a * TS];
-                b1[k] = t1[a * TS + 8];
-                if (4 * k + lc >= nca) { b0[k] = 0.0; b1[k] = 0.0; }
-                if (ntb == 1) b1[k] = 0.0;
-            }
+            for (int k = 0; k < 7; ++k) { b0[k] = t1[ta[k]]; b1[k] = ntb > 1 ? t1[ta[k] + 8] : 0.0; }
 #pragma unroll
             for (int k = 0; k < 7; ++k) live |= (__any_sync(0xffffffffu, b0[k] != 0.0 || b1[k] != 0.0) ? 1u : 0u) << k;
 #pragma unroll
@@ -271,14 +281,14 @@ __device__ __forceinline__ void hl_build_H(int la, int lb, int pure, bool neg, d
                 }
             }
             const double sgn = (neg && (s_herm[h0 + ih] >> 24 & 1)) ? -coef : coef;
+            double *hrow = dst.base + dst.row(h0 + ih);
 #pragma unroll
             for (int i = 0; i < 2; ++i)
 #pragma unroll
-                for (int n = 0; n < 2; ++n) {
-                    const int ma = 8 * i + lr, mb = 8 * n + 2 * lc;
-                    if (ma < nsa && mb < nsb) *dst(h0 + ih, ma * nsb + mb) = sgn * c[i][n][0];
-                    if (ma < nsa && mb + 1 < nsb) *dst(h0 + ih, ma * nsb + mb + 1) = sgn * c[i][n][1];
-                }
+                for (int n = 0; n < 2; ++n)
+#pragma unroll
+                    for (int e = 0; e < 2; ++e)
+                        if (hval[i][n][e]) hrow[hoff[i][n][e]] = sgn * c[i][n][e];
         }
         __syncwarp();                                       // the slice is rewritten by the warp's next group
     }
