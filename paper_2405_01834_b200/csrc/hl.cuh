@@ -44,6 +44,7 @@ struct HlArgs {
     double *scratch;                     // fused mode: [grid][scratch_stride]
     int fused;                           // 1: S1 runs inside the quartet kernel into the CTA's scratch; 0: pair records
     int by_quartet;                      // record mode: 1 = record r belongs to quartet q_begin + r, 0 = to pair r
+    int qswap;                           // 1: the kernel's bra is the CALLER's ket (index columns and product order swapped)
     const double *rec_b, *rec_k;         // record mode: H records of hl_pair_kernel (same layout as the scratch halves)
     const double *hdr_b, *hdr_k;         // record mode: {p, Px, Py, Pz} per record and primitive
     long long rec_stride_b, rec_stride_k;
@@ -392,6 +393,7 @@ struct HlPairArgs {
     long long nrec, rec_stride;
     double *rec, *hdr;                   // [nrec][rec_stride], [nrec][K1*K2][4]
     int by_quartet;                      // record r <- side of quartet q_begin + r instead of pair r
+    int qswap;
     const int32_t *qidx;
     long long q_begin, nket;
     int o_herm, o_ct, o_ws, ws_doubles;  // shared-memory carve-up (doubles)
@@ -410,8 +412,9 @@ __global__ void __launch_bounds__(128, 4) hl_pair_kernel(HlPairArgs g) {
         long long ip = r;
         if (g.by_quartet) {
             const long long q = g.q_begin + r;
-            if (g.qidx) ip = g.qidx[2 * q + g.ket];
-            else ip = g.ket ? q % g.nket : q / g.nket;
+            const int col = g.ket ^ g.qswap;                     // column of the caller's index list / product
+            if (g.qidx) ip = g.qidx[2 * q + col];
+            else ip = col ? q % g.nket : q / g.nket;
         }
         hl_side<NTHR, NT>(g.pv, g.ket != 0, g.l1, g.l2, g.K1, g.K2, g.pure, ip, g.hdr + r * 4 * g.K1 * g.K2, sm + g.o_ws,
                           g.ws_doubles, s_herm, CT, CT + 28 * MD_HL_CSTR, g.rec + r * g.rec_stride, g.nh, g.nh_pad, g.sb,
@@ -503,7 +506,8 @@ __global__ void __launch_bounds__(32 * NWARPS, (NWARPS == 4 ? 3 : 1)) hl_kernel(
 
     for (long long q = g.q_begin + blockIdx.x; q < g.q_end; q += gridDim.x) {
         long long bi, ki;
-        if (g.qidx) { bi = g.qidx[2 * q]; ki = g.qidx[2 * q + 1]; }
+        if (g.qidx) { bi = g.qidx[2 * q + g.qswap]; ki = g.qidx[2 * q + 1 - g.qswap]; }
+        else if (g.qswap) { bi = q % g.nket; ki = q / g.nket; }     // g.nket = the caller's ket count = this kernel's bra count
         else { bi = q / g.nket; ki = q % g.nket; }
         double *out = g.out + q * g.s_q + bi * g.s_bi + ki * g.s_ki;
         __syncthreads();                                   // the previous quartet is done with shared memory and the scratch

@@ -40,8 +40,36 @@ struct HlPlan {
 inline int even_up(int x) { return x + (x & 1); }
 inline int up16(int x) { return (x + 15) / 16 * 16; }
 
-bool make_plan(const HlCall &c, int nsm, HlPlan &P) {
+// Model cost of the two contractions for one orientation (Table I, columns 3 and 4, per primitive quartet / bra primitive).
+double hl_cost(int nhb, int nhk, int nab, int ncd, int Kbra, int Kket) {
+    return (double)Kbra * Kket * 2.0 * nhb * nhk * ncd + (double)Kbra * 2.0 * nab * nhb * ncd;
+}
+
+bool make_plan(const HlCall &c0, int nsm, HlPlan &P) {
     HlArgs &a = P.a;
+    // (ab|cd) = (cd|ab): the side with the cheaper contraction order becomes the kernel's bra (PAPER.md:133, 187 orders the
+    // sides for the same reason).  By measurement (profiles/r02_hl_swap.md): whenever the ket has the higher total angular
+    // momentum (1.02-1.18x on all ten pairs of orientations tried; the Table-I cost ratio predicts the sign but not the size).
+    HlCall c = c0;
+    a.qswap = 0;
+    {
+        const int pure = c0.pure;
+        auto sz = [&](const PairView &p, int &nh, int &n, int &K) {
+            const int l1 = p.a.l, l2 = p.single ? 0 : p.b.l;
+            nh = nherm(l1 + l2); n = ncomp(l1, pure) * ncomp(l2, pure); K = p.a.K * (p.single ? 1 : p.b.K);
+        };
+        int nhb, nab, Kb, nhk, ncd, Kk;
+        sz(c0.bra, nhb, nab, Kb); sz(c0.ket, nhk, ncd, Kk);
+        int mode = -1;
+        if (const char *f = getenv("MD_HL_SWAP")) mode = atoi(f);
+        (void)hl_cost;
+        const bool want = mode >= 0 ? mode != 0 : nhk > nhb;          // the side with the higher total l becomes the bra
+        if (want && !c0.ket.single && !c0.bra.single) {
+            std::swap(c.bra, c.ket);
+            std::swap(c.s_bi, c.s_ki); std::swap(c.s_ab, c.s_cd);
+            a.qswap = 1;
+        }
+    }
     a.bra = c.bra; a.ket = c.ket; a.pure = c.pure;
     a.la = c.bra.a.l; a.lb = c.bra.single ? 0 : c.bra.b.l; a.lc = c.ket.a.l; a.ld = c.ket.single ? 0 : c.ket.b.l;
     a.Ka = c.bra.a.K; a.Kb = c.bra.single ? 1 : c.bra.b.K; a.Kc = c.ket.a.K; a.Kd = c.ket.single ? 1 : c.ket.b.K;
@@ -54,7 +82,7 @@ bool make_plan(const HlCall &c, int nsm, HlPlan &P) {
     int nmt = (a.Kbra * a.nhb + 7) / 8;                   // row tiles if all bra primitives share one row block (refined below)
     a.sb = (8 * nmt2 - 4 + 15) / 16 * 16 + 4;
     a.q_first = (c.ket.single && c.pure) ? nherm(a.lc - 1) / MD_HL_KC1 * MD_HL_KC1 : 0;
-    a.qidx = c.qidx; a.nq = c.nq; a.nket = c.ket.npairs; a.out = c.out;
+    a.qidx = c.qidx; a.nq = c.nq; a.nket = c0.ket.npairs; a.out = c.out;
     a.s_q = c.s_q; a.s_bi = c.s_bi; a.s_ki = c.s_ki; a.s_ab = c.s_ab; a.s_cd = c.s_cd;
     a.boys_tab = c.boys_tab; a.rlut = c.rlut;
     const int L = a.Lb + a.Lk, nR = a.Kbra * a.Kket;
@@ -164,7 +192,7 @@ bool make_plan(const HlCall &c, int nsm, HlPlan &P) {
         g.tile_stride = side ? (long long)a.Kket * a.nhk_pad * NTS : 0;
         g.kbb = side ? 1 : a.kbb; g.blk_rows = side ? 0 : a.mrows_pad;
         g.rec_stride = side ? P.reck : P.recb;
-        g.by_quartet = mode == 2; g.qidx = c.qidx; g.nket = npk;
+        g.by_quartet = mode == 2; g.qidx = c.qidx; g.nket = c0.ket.npairs; g.qswap = a.qswap;
         const int esz = (g.l1 + 1) * (g.l2 + 1) * (g.l1 + g.l2 + 1);
         int o = 0;
         g.o_herm = o; o += nherm(g.l1 + g.l2) / 2 + 1;
@@ -202,7 +230,7 @@ cudaError_t hl_launch(const HlCall &c, int nsm, void *scratch, cudaStream_t st, 
         // record layout in the workspace: [bra records][ket records][bra headers][ket headers]; padding stays zero
         cudaError_t e = cudaMemsetAsync(scratch, 0, P.scratch_bytes, st);
         if (e != cudaSuccess) return e;
-        const long long nrb = P.mode == 1 ? c.bra.npairs : P.chunk, nrk = P.mode == 1 ? c.ket.npairs : P.chunk;
+        const long long nrb = P.mode == 1 ? P.pb.pv.npairs : P.chunk, nrk = P.mode == 1 ? P.pk.pv.npairs : P.chunk;   // kernel's sides (maybe swapped)
         double *recb = (double *)scratch, *reck = recb + nrb * P.recb;
         double *hdrb = reck + nrk * P.reck, *hdrk = hdrb + nrb * 4 * a.Kbra;
         a.rec_b = recb; a.rec_k = reck; a.hdr_b = hdrb; a.hdr_k = hdrk;
