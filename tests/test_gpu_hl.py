@@ -83,3 +83,17 @@ def test_hl_chunked_launches(mode):
 def test_hl_ragged_counts(mode):
     for n in (1, 2, 147, 149, 297):
         check(W.class_sweep((3, 3, 2, 1), n), True, HL, sel=np.arange(0, n, max(1, n // 20)))
+
+
+def test_hl_either_orientation(mode):
+    """(ab|cd) = (cd|ab): the kernel may take the caller's ket as its bra (MD_HL_SWAP forces either choice)."""
+    try:
+        for sw in ("0", "1"):
+            os.environ["MD_HL_SWAP"] = sw
+            for ls in [(3, 2, 4, 1), (4, 4, 3, 3), (1, 0, 4, 3)]:
+                check(W.class_sweep(ls, 19), True, HL)
+                check(W.class_sweep(ls, 19), False, HL)
+            check(W.paper_microbench((3, 2, 4, 1), 1, 2, 9, 7), True, HL)
+            check(W.independent_quartets("sw", (3, 1, 2, 2), (2, 1, 1, 3), 31, (0.05, 50.0), (-2.0, 2.0), 3), True, HL)
+    finally:
+        os.environ.pop("MD_HL_SWAP", None)
