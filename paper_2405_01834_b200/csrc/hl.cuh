@@ -584,55 +584,68 @@ __global__ void __launch_bounds__(32 * NWARPS, (NWARPS == 4 ? 3 : 1)) hl_kernel(
                 for (int n = 0; n < NW; ++n) c2[t][n][0] = c2[t][n][1] = 0.0;
             for (int blk = 0; blk < g.nblk; ++blk) {
             // GEMM1 (Eqs. 19, 25): rows = stacked (kb, p~) of the row block, columns = this cd tile, K = (kk, q~)
-            for (int pass = 0; pass < npass; ++pass) {
-                uint32_t wrow[MW];
-                int rbase[MW];
+            // One row pass, specialised on the number of row tiles this warp really owns in it (the last pass is ragged):
+            // no tensor-core step is spent on tiles past the end, and the inner loop stays branch-free.
+            auto gemm1_pass = [&](auto mwc, int pass) {
+                constexpr int MWc = decltype(mwc)::value, MWa = MWc > 0 ? MWc : 1;
+                uint32_t wrow[MWa];
+                int rbase[MWa];
 #pragma unroll
-                for (int i = 0; i < MW; ++i) {                 // row tiles past the end compute on a clamped row; not stored
+                for (int i = 0; i < MWc; ++i) {
                     const int mt = (pass * MW + i) * NWARPS + warp;
-                    const int2 ri = rowinfo[min(mt, nmt - 1) * 8 + lr];
+                    const int2 ri = rowinfo[mt * 8 + lr];
                     wrow[i] = (uint32_t)ri.x; rbase[i] = min(blk * g.kbb + ri.y, g.Kbra - 1) * g.rs0;
                 }
-                double acc[MW][NW][2];
+                double acc[MWa][NW][2];
 #pragma unroll
-                for (int i = 0; i < MW; ++i)
+                for (int i = 0; i < MWa; ++i)
 #pragma unroll
                     for (int n = 0; n < NW; ++n) acc[i][n][0] = acc[i][n][1] = 0.0;
                 for (int kk = 0; kk < g.Kket; ++kk) {
                     const double *Rk = R0 + (long long)kk * g.Kbra * g.rs0;
                     for (int c = c_first; c < nc1; ++c) {
                         const double *B = acquire() + lc * NTS + lr;
-                        const int q0 = c * MD_HL_KC1 + lc;
-                        const int nsteps = min(MD_HL_KC1 / 4, (nhk - c * MD_HL_KC1 + 3) >> 2);   // rows >= nhk of Hk are zero
-                        if (nsteps == MD_HL_KC1 / 4) {
-                            uint32_t wq[MD_HL_KC1 / 4];
+                        if (MWc > 0) {
+                            const int q0 = c * MD_HL_KC1 + lc;
+                            const int nsteps = min(MD_HL_KC1 / 4, (nhk - c * MD_HL_KC1 + 3) >> 2);   // rows >= nhk of Hk are zero
+                            if (nsteps == MD_HL_KC1 / 4) {
+                                uint32_t wq[MD_HL_KC1 / 4];
 #pragma unroll
-                            for (int k = 0; k < MD_HL_KC1 / 4; ++k) wq[k] = s_herm[min(q0 + 4 * k, nhk - 1)];
-                            if (nnt == NW) {
+                                for (int k = 0; k < MD_HL_KC1 / 4; ++k) wq[k] = s_herm[min(q0 + 4 * k, nhk - 1)];
+                                if (nnt == NW) {
 #pragma unroll
-                                for (int k = 0; k < MD_HL_KC1 / 4; ++k)
-                                    hl_gemm1_step<MW, NW, true>(acc, B + 4 * k * NTS, Rk, rbase, wrow, wq[k], nnt);
+                                    for (int k = 0; k < MD_HL_KC1 / 4; ++k)
+                                        hl_gemm1_step<MWa, NW, true>(acc, B + 4 * k * NTS, Rk, rbase, wrow, wq[k], nnt);
+                                } else {
+#pragma unroll
+                                    for (int k = 0; k < MD_HL_KC1 / 4; ++k)
+                                        hl_gemm1_step<MWa, NW, false>(acc, B + 4 * k * NTS, Rk, rbase, wrow, wq[k], nnt);
+                                }
                             } else {
-#pragma unroll
-                                for (int k = 0; k < MD_HL_KC1 / 4; ++k)
-                                    hl_gemm1_step<MW, NW, false>(acc, B + 4 * k * NTS, Rk, rbase, wrow, wq[k], nnt);
+                                for (int k = 0; k < nsteps; ++k)
+                                    hl_gemm1_step<MWa, NW, false>(acc, B + 4 * k * NTS, Rk, rbase, wrow, s_herm[min(q0 + 4 * k, nhk - 1)], nnt);
                             }
-                        } else {
-                            for (int k = 0; k < nsteps; ++k)
-                                hl_gemm1_step<MW, NW, false>(acc, B + 4 * k * NTS, Rk, rbase, wrow, s_herm[min(q0 + 4 * k, nhk - 1)], nnt);
                         }
                         release();
                     }
                 }
 #pragma unroll
-                for (int i = 0; i < MW; ++i) {
+                for (int i = 0; i < MWc; ++i) {
                     const int mt = (pass * MW + i) * NWARPS + warp;
-                    if (mt < nmt) {
 #pragma unroll
-                        for (int n = 0; n < NW; ++n)
-                            *(double2 *)(Vp + (mt * 8 + lr) * NTS + n * 8 + 2 * lc) = make_double2(acc[i][n][0], acc[i][n][1]);
-                    }
+                    for (int n = 0; n < NW; ++n)
+                        *(double2 *)(Vp + (mt * 8 + lr) * NTS + n * 8 + 2 * lc) = make_double2(acc[i][n][0], acc[i][n][1]);
                 }
+            };
+            for (int pass = 0; pass < npass; ++pass) {
+                const int left_tiles = nmt - pass * MW * NWARPS - warp;      // this warp owns tiles warp, warp + NWARPS, .. of the pass
+                const int mine = left_tiles <= 0 ? 0 : min(MW, (left_tiles + NWARPS - 1) / NWARPS);
+                using std::integral_constant;
+                if (mine == MW) gemm1_pass(integral_constant<int, MW>{}, pass);
+                else if (MW > 3 && mine == 3) gemm1_pass(integral_constant<int, (MW > 3 ? 3 : 0)>{}, pass);
+                else if (MW > 2 && mine == 2) gemm1_pass(integral_constant<int, (MW > 2 ? 2 : 0)>{}, pass);
+                else if (MW > 1 && mine == 1) gemm1_pass(integral_constant<int, (MW > 1 ? 1 : 0)>{}, pass);
+                else gemm1_pass(integral_constant<int, 0>{}, pass);
             }
             __syncthreads();
             // GEMM2 (Eq. 26): rows = ab (MD_HL_MT2 tiles per warp), columns = the cd tile, K = stacked (kb, p~)

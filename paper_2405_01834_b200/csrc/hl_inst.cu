@@ -98,9 +98,13 @@ bool make_plan(const HlCall &c0, int nsm, HlPlan &P) {
     warps = (nmt <= 12 && nmt2 <= 4 * MD_HL_MT2) ? 4 : 8;
     MW = 1;
     double best = 1e30;
-    for (int m = 1; m <= (warps == 4 ? 3 : 4); ++m) {     // tile slots, weighted by the operand traffic per tensor-core step
-        const double cost = (nmt + warps * m - 1) / (warps * m) * m * (1.0 + 0.35 / m);
-        if (cost < best) { best = cost; MW = m; }
+    for (int m = 1; m <= (warps == 4 ? 3 : 4); ++m) {     // critical path in row-tile passes (a ragged last pass only costs the
+        double cost = 0;                                   // tiles it has), weighted by the operand traffic per tensor-core step
+        for (int left = nmt; left > 0; left -= warps * m) {
+            const int t = (std::min(left, warps * m) + warps - 1) / warps;
+            cost += t * (1.0 + 0.35 / t);
+        }
+        if (cost <= best) { best = cost; MW = m; }
     }
     if (const char *f = getenv("MD_HL_FORCE")) {           // measurement override: "MW,NW,warps"
         int m, n, w;
