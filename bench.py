@@ -174,7 +174,7 @@ def measure_variant(dw, w, K, pure, steps, warmup, flush, barrier):
 
 
 
-VARIANT_NAME = {1: "generic", 2: "fused", 3: "mma", 4: "fused2", 5: "warp", 6: "hl", 7: "lowl"}
+VARIANT_NAME = {1: "generic", 2: "fused", 3: "mma", 4: "fused2", 5: "warp", 6: "hl", 7: "lowl", 8: "eri3s"}
 
 
 def per_class_cases():
@@ -550,7 +550,7 @@ def run_autotune(args):
     engine.md_init()
     os.environ["MD_NO_TABLE"] = "1"                       # candidates are forced explicitly; AUTO below means the RULES
     flush = torch.empty(256 << 20, dtype=torch.uint8, device="cuda")
-    vid = {"rules": 0, "generic": 1, "fused": 2, "mma": 3, "fused2": 4, "warp": 5, "hl": 6, "lowl": 7}
+    vid = {"rules": 0, "generic": 1, "fused": 2, "mma": 3, "fused2": 4, "warp": 5, "hl": 6, "lowl": 7, "eri3s": 8}
     pairs = [(a, b) for a in range(7) for b in range(a + 1)]
     cases = []
     for ib, b in enumerate(pairs):
@@ -575,8 +575,10 @@ def run_autotune(args):
                 w = W.independent_quartets("at", ls, K, n, (0.3, 10.0), (-4.0, 4.0), W.class_seed("at", ls, contracted), three_center=three)
                 if lmax <= 1:
                     cands = ["lowl", "fused", "fused2"]
-                elif lmax <= 2:
+                elif lmax <= 2 and not three:
                     cands = ["fused", "fused2"]
+                elif three and max(ls[0], ls[1]) <= 3:
+                    cands = ["eri3s", "warp", "mma", "hl"] if lmax > 2 else ["eri3s", "fused", "fused2"]
                 else:
                     cands = ["warp", "mma", "hl"]
                 dw = engine.DeviceWorkload(w); out = dw.alloc_out(True)
@@ -628,7 +630,7 @@ def run_sweep(args):
     engine.md_init()
     flush = torch.empty(256 << 20, dtype=torch.uint8, device="cuda")
     vid = {"auto": engine.VARIANT_AUTO, "generic": engine.VARIANT_GENERIC, "fused": engine.VARIANT_FUSED,
-           "mma": engine.VARIANT_MMA, "fused2": engine.VARIANT_FUSED2, "warp": engine.VARIANT_WARP, "hl": engine.VARIANT_HL, "lowl": engine.VARIANT_LOWL}
+           "mma": engine.VARIANT_MMA, "fused2": engine.VARIANT_FUSED2, "warp": engine.VARIANT_WARP, "hl": engine.VARIANT_HL, "lowl": engine.VARIANT_LOWL, "eri3s": engine.VARIANT_ERI3S}
     vname = VARIANT_NAME
     try:
         hbm = json.load(open(os.path.join(ROOT, "MEASURED_PEAKS.json"))).get("hbm_gbs", 6550.0)

@@ -199,6 +199,7 @@ int md_set_workspace(void *device_ptr, size_t bytes);
 #define MD_VARIANT_WARP    5     /* pair setup + the one-warp-per-quartet kernel where the class is small enough, else as MMA */
 #define MD_VARIANT_HL     6     /* the one-launch high-l kernel (in-kernel pair setup, TMA-staged DMMA) where it fits, else as MMA */
 #define MD_VARIANT_LOWL   7     /* one thread per quartet, registers only, for classes with every l <= 1 (quartet-major layout), else as AUTO */
+#define MD_VARIANT_ERI3S  8     /* one warp per triplet, sparse Cartesian bra, for 3-center classes with la, lb <= 3, else as AUTO */
 int md_set_variant(int variant);
 /* Which variant the last md_eri4/md_eri3 call used (MD_VARIANT_GENERIC, _FUSED, _MMA, _FUSED2 or _WARP),
  * and how many kernels it launched. */

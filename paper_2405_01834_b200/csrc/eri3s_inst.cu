@@ -1,0 +1,56 @@
+// eri3s_inst.cu -- host side of the one-warp-per-triplet 3-center kernel (eri3s.cuh).
+#include <algorithm>
+
+#include "eri3s.cuh"
+#include "eri3s_api.cuh"
+
+namespace mdb {
+
+namespace { int g_e3_max_smem = 227 * 1024; }
+
+cudaError_t eri3s_init(int max_smem, const uint32_t *herm, const double *solid) {
+    g_e3_max_smem = max_smem;
+    cudaError_t e = upload_tables(herm, solid);
+    if (e != cudaSuccess) return e;
+    return cudaFuncSetAttribute(eri3s_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, max_smem);
+}
+
+bool eri3s_has_class(const PairView &b, const PairView &k) {
+    return k.single && !b.single && b.a.l <= 3 && b.b.l <= 3;
+}
+
+int eri3s_dispatch(const PairView &b, const PairView &k, long long nt, const int32_t *tidx, int pure, double *out,
+                   const double *boys_tab, const uint32_t *rlut, int nsm, cudaStream_t st) {
+    if (!eri3s_has_class(b, k)) return 0;
+    Eri3sArgs g;
+    g.bra = b; g.X = k.a; g.pure = pure;
+    g.la = b.a.l; g.lb = b.b.l; g.lX = k.a.l; g.Ka = b.a.K; g.Kb = b.b.K; g.KX = k.a.K;
+    g.nca = ncart(g.la); g.ncb = ncart(g.lb); g.nXc = ncomp(g.lX, pure);
+    g.nhb = nherm(g.la + g.lb); g.L = g.la + g.lb + g.lX;
+    g.tidx = tidx; g.nt = nt; g.nX = k.npairs; g.out = out; g.boys_tab = boys_tab; g.rlut = rlut;
+    auto even = [](int x) { return x + (x & 1); };
+    int o = 0;
+    g.o_r0 = o; o += even(nherm(g.L));
+    g.o_r1 = o; o += even(g.L > 0 ? nherm(g.L - 1) : 1);
+    g.o_g = o; o += even(g.nhb * g.nXc);
+    g.o_acc = o; o += even(g.nca * g.ncb * g.nXc);
+    g.o_e = o; o += even(3 * (g.la + 1) * (g.lb + 1) * (g.la + g.lb + 1));
+    g.o_ex = o; o += even((g.lX + 1) * (g.lX + 1));
+    g.o_g0 = o; o += even(g.L + 1);
+    g.per_warp = o;
+    const size_t fixed = 8 * (228 + 4 * 28 * MD_HL_CSTR + 88);   // Hermite triples, four transposed solid tables, the (t,u,v) cube
+    const size_t avail = (size_t)g_e3_max_smem - fixed;
+    int warps = (int)std::min<size_t>(8, avail / (8 * (size_t)o));
+    if (warps < 1) return 0;
+    // several CTAs per SM when the slices are small: the warps of one CTA share nothing but the constant tables
+    int threads = warps > 4 ? 256 : 128;
+    if (warps == 8 && fixed + 8 * (size_t)o * 4 <= (size_t)g_e3_max_smem / 4) { warps = 4; threads = 128; }   // 4 CTAs of 4 warps
+    g.warps = warps;
+    const size_t smem = fixed + 8 * (size_t)o * warps;
+    const int ctas = (int)std::max<size_t>(1, std::min<size_t>(2048 / threads, (size_t)(g_e3_max_smem + 1024) / (smem + 1024)));
+    const long long nblk = (nt + warps - 1) / warps;
+    eri3s_kernel<<<(unsigned)std::min<long long>(nblk, (long long)nsm * ctas), threads, smem, st>>>(g);
+    return 1;
+}
+
+}  // namespace mdb

@@ -17,6 +17,7 @@
 #include "generic.cuh"
 #include "hl_api.cuh"
 #include "lowl_api.cuh"
+#include "eri3s_api.cuh"
 #include "mma_api.cuh"
 #include "pair.cuh"
 #include "warp.cuh"
@@ -361,6 +362,18 @@ int run_rules(const PairView &b, const PairView &k, long long nq, const int32_t 
             return MD_OK;
         }
     }
+    // 3-center with la, lb <= 3 (BASELINE configs[2]): one warp per triplet in the sparse Cartesian form (eri3s.cuh); by
+    // measurement (profiles/r02_eri3s.md) under AUTO for every such class that has an l >= 2 shell.
+    if ((S.variant == MD_VARIANT_ERI3S || (S.variant == MD_VARIANT_AUTO && std::max({s.la, s.lb, s.lc}) >= 2)) &&
+        layout == MD_LAYOUT_QUARTET_MAJOR && eri3s_has_class(b, k)) {
+        if (sc.dry) { sc.need = 0; return MD_DRY; }
+        if (eri3s_dispatch(b, k, nq, qidx, pure, out, S.boys_tab, fused_rlut(), S.nsm, st) == 1) {
+            S.last_launches++;
+            CK(cudaGetLastError());
+            S.last_variant = MD_VARIANT_ERI3S;
+            return MD_OK;
+        }
+    }
     if (S.variant == MD_VARIANT_AUTO || S.variant == MD_VARIANT_FUSED2) {
         // By measurement (profiles/r01_sweep_l2.md): the warp-specialised kernel wins on every instantiated class
         // once the primitive loop is long enough to fill its pipeline, and on (dd|dd) for any K.
@@ -568,6 +581,7 @@ int md_init(void) {
     CK(mma_init(S.max_smem));
     CK(hl_init(S.max_smem, herm.data(), solid.data()));
     CK(lowl_init(S.max_smem));
+    CK(eri3s_init(S.max_smem, herm.data(), solid.data()));
     CK(cudaDeviceSynchronize());
     S.init = true;
     S.device = dev;
@@ -656,7 +670,7 @@ int md_set_workspace(void *p, size_t bytes) {
     return MD_OK;
 }
 int md_set_variant(int v) {
-    if (v < MD_VARIANT_AUTO || v > MD_VARIANT_LOWL) return MD_EINVAL;
+    if (v < MD_VARIANT_AUTO || v > MD_VARIANT_ERI3S) return MD_EINVAL;
     S.variant = v;
     return MD_OK;
 }

@@ -12,7 +12,7 @@ LIB_PATH = os.path.join(_HERE, "libmdb200.so")
 
 MD_OK, MD_EINVAL, MD_ECAPACITY, MD_ECUDA, MD_ENOMEM = 0, -1, -2, -3, -4
 LAYOUT_QUARTET_MAJOR, LAYOUT_PAPER = 0, 1
-VARIANT_AUTO, VARIANT_GENERIC, VARIANT_FUSED, VARIANT_MMA, VARIANT_FUSED2, VARIANT_WARP, VARIANT_HL, VARIANT_LOWL = 0, 1, 2, 3, 4, 5, 6, 7
+VARIANT_AUTO, VARIANT_GENERIC, VARIANT_FUSED, VARIANT_MMA, VARIANT_FUSED2, VARIANT_WARP, VARIANT_HL, VARIANT_LOWL, VARIANT_ERI3S = 0, 1, 2, 3, 4, 5, 6, 7, 8
 
 _dp = ctypes.POINTER(ctypes.c_double)
 _ip = ctypes.POINTER(ctypes.c_int32)
