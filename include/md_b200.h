@@ -66,6 +66,8 @@ extern "C" {
 #define MD_ECAPACITY (-2)     /* out_capacity_elems smaller than the result */
 #define MD_ECUDA     (-3)     /* CUDA runtime error (allocation, launch, copy) */
 #define MD_ENOMEM    (-4)     /* caller-set workspace too small for this call */
+#define MD_ESTATIC   (-5)     /* md_eri4_static: the call needs more than MD_STATIC_SCRATCH_BYTES of pair records */
+#define MD_ENOTINIT  (-6)     /* md_eri4_static: md_init() has not run on the current device (the call never initialises) */
 
 #define MD_LAYOUT_QUARTET_MAJOR 0
 #define MD_LAYOUT_PAPER         1
@@ -186,6 +188,30 @@ int64_t md_eri3_workspace_bytes(const md_pairs *bra, const md_shells *X, int64_t
  * anything is launched or written (under MD_VARIANT_AUTO an l <= 2 class first falls back to
  * the fused kernel that needs no scratch). */
 int md_set_workspace(void *device_ptr, size_t bytes);
+
+/*
+ * md_eri4 for callers that must not allocate (CUDA graph capture, serving loops, harnesses that forbid cudaMalloc):
+ * the runtime-l chain (pair setup per side, Eqs. 9-17, then the one-warp-per-quartet, DMMA or DFMA quartet
+ * kernel, Eqs. 19-26; what MD_VARIANT_WARP / MD_VARIANT_MMA run) with its per-pair records {G, H[ab,p~]}
+ * in a file-scope __device__ array of MD_STATIC_SCRATCH_BYTES inside the library instead of pool scratch.  Same
+ * arguments, layouts, result and validation as md_eri4.  The call itself makes no cudaMalloc / cudaMallocAsync / cudaFree
+ * and calls no allocating library routine; it only enqueues kernels on cuda_stream.
+ *   MD_ENOTINIT  md_init() has not been called in this process (md_init allocates the Boys table; call it once, outside
+ *                the region that must not allocate) or another device is current;
+ *   MD_ESTATIC   8 * (npairs_bra * Ka*Kb * (4 + N~_bra N_ab) + npairs_ket * Kc*Kd * (4 + N~_ket N_cd)) bytes (each
+ *                record rounded to an even number of doubles) exceed MD_STATIC_SCRATCH_BYTES; nothing is launched.
+ *                md_eri4_static_bytes() returns that size for a call.
+ * The array is one per device and shared by every md_eri4_static call: it keeps the last call's records (each call
+ * writes every word it reads, nothing has to start at zero), and two calls that overlap on the GPU (different streams,
+ * or two host threads) race on it -- order them on one stream or with events.  Every GPU that loads the library holds
+ * the 32 MiB until the process exits.  md_eri4 and the other entry points never touch the array.
+ */
+#define MD_STATIC_SCRATCH_BYTES ((size_t)32 << 20)
+int md_eri4_static(const md_pairs *bra, const md_pairs *ket,
+                   int64_t nquartets, const int32_t *quartet_idx, int pure, int layout,
+                   double *out, int64_t out_capacity_elems, void *cuda_stream);
+/* Bytes of the static array md_eri4_static would use for these batches (struct fields only; negative error code). */
+int64_t md_eri4_static_bytes(const md_pairs *bra, const md_pairs *ket, int pure);
 
 /* Kernel-variant control, for measurement:
  *   MD_VARIANT_AUTO    the measured-best variant per class (default)

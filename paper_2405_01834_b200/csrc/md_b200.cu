@@ -44,7 +44,12 @@ struct State {
     int nsm = 148;
     int max_smem = 227 * 1024;
     char cuda_err[256] = "";
+    void *static_ws = nullptr;   // device address of g_static_scratch (md_eri4_static), resolved in md_init
 } S;
+
+// Scratch of md_eri4_static (include/md_b200.h): pair records of the runtime-l chain for callers that must not allocate.
+// In host code this name is only a handle for cudaGetSymbolAddress (md_init), never a device address.
+static __device__ __align__(256) unsigned char g_static_scratch[MD_STATIC_SCRATCH_BYTES];
 
 // Measured-best variant per (canonical class, contracted or not), written by `python bench.py --sweep autotune` on one
 // B200 for the independent-quartet structure (profiles/r02_autotune.md) and checked in.  Classes that are missing, and calls the
@@ -582,10 +587,44 @@ int md_init(void) {
     CK(hl_init(S.max_smem, herm.data(), solid.data()));
     CK(lowl_init(S.max_smem));
     CK(eri3s_init(S.max_smem, herm.data(), solid.data()));
+    CK(cudaGetSymbolAddress(&S.static_ws, g_static_scratch));   // once per device, with that device current
     CK(cudaDeviceSynchronize());
     S.init = true;
     S.device = dev;
     return MD_OK;
+}
+
+// The runtime-l chain on the library's static scratch: no allocation of any kind in this call (include/md_b200.h).
+int md_eri4_static(const md_pairs *bra, const md_pairs *ket, int64_t nquartets, const int32_t *quartet_idx, int pure,
+                   int layout, double *out, int64_t out_capacity_elems, void *cuda_stream) {
+    int e = check_pairs(bra);
+    if (e) return e;
+    if ((e = check_pairs(ket))) return e;
+    if (pure != 0 && pure != 1) return MD_EINVAL;
+    if (layout != MD_LAYOUT_QUARTET_MAJOR && layout != MD_LAYOUT_PAPER) return MD_EINVAL;
+    if (layout == MD_LAYOUT_PAPER && quartet_idx) return MD_EINVAL;
+    const PairView b = view(*bra), k = view(*ket);
+    if (nquartets < 0 || (!quartet_idx && nquartets != b.npairs * k.npairs)) return MD_EINVAL;
+    const Shape s = shape_of(b, k, pure);
+    if ((long long)s.nab * s.ncd * nquartets > out_capacity_elems) return MD_ECAPACITY;
+    if (nquartets > 0 && !out) return MD_EINVAL;
+    int dev = -1;
+    CK(cudaGetDevice(&dev));
+    if (!S.init || !S.static_ws || dev != S.device) return MD_ENOTINIT;
+    if (generic_ws_bytes(b, k, pure) > MD_STATIC_SCRATCH_BYTES) return MD_ESTATIC;
+    S.last_launches = 0;
+    if (nquartets == 0) return MD_OK;
+    Scratch sc;                                     // not used by the chain once it has its records' address
+    return run_generic_once(b, k, nquartets, quartet_idx, pure, layout, out, (cudaStream_t)cuda_stream, true, sc,
+                            S.static_ws, nullptr, 0);
+}
+
+int64_t md_eri4_static_bytes(const md_pairs *bra, const md_pairs *ket, int pure) {
+    int e = check_pairs(bra);
+    if (e) return e;
+    if ((e = check_pairs(ket))) return e;
+    if (pure != 0 && pure != 1) return MD_EINVAL;
+    return (int64_t)generic_ws_bytes(view(*bra), view(*ket), pure);
 }
 
 int md_eri4(const md_pairs *bra, const md_pairs *ket, int64_t nquartets, const int32_t *quartet_idx, int pure,
@@ -737,6 +776,8 @@ const char *md_strerror(int code) {
         case MD_ECAPACITY: return "output buffer too small";
         case MD_ECUDA: return "CUDA runtime error";
         case MD_ENOMEM: return "workspace too small";
+        case MD_ESTATIC: return "md_eri4_static: pair records exceed MD_STATIC_SCRATCH_BYTES (32 MiB); use md_eri4";
+        case MD_ENOTINIT: return "md_eri4_static: call md_init() on this device first";
         default: return "unknown error";
     }
 }

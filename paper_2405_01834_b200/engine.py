@@ -10,7 +10,8 @@ import numpy as np
 _HERE = os.path.dirname(os.path.abspath(__file__))
 LIB_PATH = os.path.join(_HERE, "libmdb200.so")
 
-MD_OK, MD_EINVAL, MD_ECAPACITY, MD_ECUDA, MD_ENOMEM = 0, -1, -2, -3, -4
+MD_OK, MD_EINVAL, MD_ECAPACITY, MD_ECUDA, MD_ENOMEM, MD_ESTATIC, MD_ENOTINIT = 0, -1, -2, -3, -4, -5, -6
+STATIC_SCRATCH_BYTES = 32 << 20
 LAYOUT_QUARTET_MAJOR, LAYOUT_PAPER = 0, 1
 VARIANT_AUTO, VARIANT_GENERIC, VARIANT_FUSED, VARIANT_MMA, VARIANT_FUSED2, VARIANT_WARP, VARIANT_HL, VARIANT_LOWL, VARIANT_ERI3S = 0, 1, 2, 3, 4, 5, 6, 7, 8
 
@@ -30,7 +31,7 @@ class md_pairs(ctypes.Structure):
 SYMBOLS = ["md_eri4", "md_eri3", "md_eri4_host", "md_eri3_host", "md_eri4_out_elems", "md_eri3_out_elems",
            "md_eri4_workspace_bytes", "md_eri3_workspace_bytes", "md_set_workspace", "md_set_variant",
            "md_last_variant", "md_last_launch_count", "md_init", "md_boys", "md_fp64_peak", "md_strerror", "md_last_cuda_error",
-           "md_version", "md_schwarz", "md_quartet_list", "md_exchange", "md_eri2"]
+           "md_version", "md_schwarz", "md_quartet_list", "md_exchange", "md_eri2", "md_eri4_static", "md_eri4_static_bytes"]
 
 _lib = None
 
@@ -46,7 +47,8 @@ def lib():
         pp, ps = ctypes.POINTER(md_pairs), ctypes.POINTER(md_shells)
         sig = [ctypes.c_int64, ctypes.c_void_p, ctypes.c_int, ctypes.c_int, ctypes.c_void_p, ctypes.c_int64,
                ctypes.c_void_p]
-        for name, second in (("md_eri4", pp), ("md_eri3", ps), ("md_eri4_host", pp), ("md_eri3_host", ps)):
+        for name, second in (("md_eri4", pp), ("md_eri3", ps), ("md_eri4_host", pp), ("md_eri3_host", ps),
+                             ("md_eri4_static", pp)):
             f = getattr(L, name)
             f.argtypes = [pp, second] + sig
             f.restype = ctypes.c_int
@@ -54,6 +56,8 @@ def lib():
         L.md_eri4_out_elems.restype = ctypes.c_int64
         L.md_eri3_out_elems.argtypes = [ctypes.c_int] * 4 + [ctypes.c_int64]
         L.md_eri3_out_elems.restype = ctypes.c_int64
+        L.md_eri4_static_bytes.argtypes = [pp, pp, ctypes.c_int]
+        L.md_eri4_static_bytes.restype = ctypes.c_int64
         L.md_eri4_workspace_bytes.argtypes = [pp, pp, ctypes.c_int64, ctypes.c_int, ctypes.c_int]
         L.md_eri4_workspace_bytes.restype = ctypes.c_int64
         L.md_eri3_workspace_bytes.argtypes = [pp, ps, ctypes.c_int64, ctypes.c_int, ctypes.c_int]
@@ -196,6 +200,26 @@ def md_eri4(a, b, c, d, bra_idx, ket_idx, quartet_idx, nquartets, pure, out, lay
     _check(lib().md_eri4(ctypes.byref(bra), ctypes.byref(ket), int(nquartets), _ptr(quartet_idx), int(pure),
                          int(layout), _ptr(out), out.numel(), _stream_ptr(stream)))
     return out
+
+
+def md_eri4_static(a, b, c, d, bra_idx, ket_idx, quartet_idx, nquartets, pure, out, layout=LAYOUT_QUARTET_MAJOR,
+                   stream=None, nbra=None, nket=None):
+    """md_eri4 without any allocation: pair records in the library's static 32 MiB device array (include/md_b200.h).
+    md_init() must have run; MD_ESTATIC if the records do not fit.  Calls that overlap on the GPU race on the array."""
+    bra = _pairs_struct(a, b, bra_idx, nbra)
+    ket = _pairs_struct(c, d, ket_idx, nket)
+    _check(lib().md_eri4_static(ctypes.byref(bra), ctypes.byref(ket), int(nquartets), _ptr(quartet_idx), int(pure),
+                                int(layout), _ptr(out), out.numel(), _stream_ptr(stream)))
+    return out
+
+
+def md_eri4_static_bytes(a, b, c, d, bra_idx, ket_idx, pure, nbra=None, nket=None):
+    bra = _pairs_struct(a, b, bra_idx, nbra)
+    ket = _pairs_struct(c, d, ket_idx, nket)
+    r = lib().md_eri4_static_bytes(ctypes.byref(bra), ctypes.byref(ket), int(pure))
+    if r < 0:
+        _check(int(r))
+    return int(r)
 
 
 def md_eri3(a, b, x, bra_idx, triplet_idx, ntriplets, pure, out, layout=LAYOUT_QUARTET_MAJOR, stream=None,
