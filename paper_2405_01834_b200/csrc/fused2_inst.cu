@@ -17,22 +17,9 @@ F2Entry *f2_table() { return g_f2; }
 cudaError_t fused2_init(int max_smem) {
     g_f2_max_smem = max_smem;
     cudaError_t e;
-    if ((e = fused2_register_11_11(max_smem)) != cudaSuccess) return e;
-    if ((e = fused2_register_11_20(max_smem)) != cudaSuccess) return e;
-    if ((e = fused2_register_11_21(max_smem)) != cudaSuccess) return e;
-    if ((e = fused2_register_11_22(max_smem)) != cudaSuccess) return e;
-    if ((e = fused2_register_20_11(max_smem)) != cudaSuccess) return e;
-    if ((e = fused2_register_20_20(max_smem)) != cudaSuccess) return e;
-    if ((e = fused2_register_20_21(max_smem)) != cudaSuccess) return e;
-    if ((e = fused2_register_20_22(max_smem)) != cudaSuccess) return e;
-    if ((e = fused2_register_21_11(max_smem)) != cudaSuccess) return e;
-    if ((e = fused2_register_21_20(max_smem)) != cudaSuccess) return e;
-    if ((e = fused2_register_21_21(max_smem)) != cudaSuccess) return e;
-    if ((e = fused2_register_21_22(max_smem)) != cudaSuccess) return e;
-    if ((e = fused2_register_22_11(max_smem)) != cudaSuccess) return e;
-    if ((e = fused2_register_22_20(max_smem)) != cudaSuccess) return e;
-    if ((e = fused2_register_22_21(max_smem)) != cudaSuccess) return e;
-    if ((e = fused2_register_22_22(max_smem)) != cudaSuccess) return e;
+#define F2_CLASS(la, lb, lc, ld) if ((e = fused2_register_##la##lb##_##lc##ld(max_smem)) != cudaSuccess) return e;
+#include "fused2_classes.inc"
+#undef F2_CLASS
     return cudaSuccess;
 }
 

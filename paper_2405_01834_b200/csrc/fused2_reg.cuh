@@ -1,5 +1,5 @@
 // fused2_reg.cuh -- registry of the warp-specialised fused kernels; one translation unit per bra pair
-// instantiates its classes (fused2_inst_*.cu), fused2_inst.cu holds the table and the launch logic.
+// instantiates its classes (generated from fused2_classes.inc by build.py), fused2_inst.cu holds the table and the launch logic.
 #pragma once
 #include "fused2_main.cuh"
 
@@ -36,22 +36,9 @@ cudaError_t f2_reg(int max_smem) {
     return cudaSuccess;
 }
 
-// one registration function per class, each in its own translation unit (fused2_inst_<bra>_<ket>.cu)
-cudaError_t fused2_register_11_11(int max_smem);
-cudaError_t fused2_register_11_20(int max_smem);
-cudaError_t fused2_register_11_21(int max_smem);
-cudaError_t fused2_register_11_22(int max_smem);
-cudaError_t fused2_register_20_11(int max_smem);
-cudaError_t fused2_register_20_20(int max_smem);
-cudaError_t fused2_register_20_21(int max_smem);
-cudaError_t fused2_register_20_22(int max_smem);
-cudaError_t fused2_register_21_11(int max_smem);
-cudaError_t fused2_register_21_20(int max_smem);
-cudaError_t fused2_register_21_21(int max_smem);
-cudaError_t fused2_register_21_22(int max_smem);
-cudaError_t fused2_register_22_11(int max_smem);
-cudaError_t fused2_register_22_20(int max_smem);
-cudaError_t fused2_register_22_21(int max_smem);
-cudaError_t fused2_register_22_22(int max_smem);
+// one registration function per class, each in its own generated translation unit (fused2_classes.inc, build.py)
+#define F2_CLASS(la, lb, lc, ld) cudaError_t fused2_register_##la##lb##_##lc##ld(int max_smem);
+#include "fused2_classes.inc"
+#undef F2_CLASS
 
 }  // namespace mdb
