@@ -20,6 +20,7 @@
 // (Eq. 16), applies Eq. 26 ([ab|cd] += sum_p~ E^{ab}_{p~} [p~|cd]) with the bra transform, and
 // accumulates into the output block, which stays in L2 between bra primitives.
 #pragma once
+#include <cuda_pipeline.h>
 #include "boys.cuh"
 #include "fused2_tables.cuh"
 #include "fused_kernel.cuh"      // axis_table, solid2, FusedArgs
@@ -66,8 +67,16 @@ struct F2Cfg {
     static_assert(O_EPB <= 2 * CB, "the [p~|cd] rows must fit in the two buffers of one producer group");
     // per quartet, never aliased: shell indices, output base
     static constexpr int PERQ = 4;
-    static constexpr int QTOT = PERQ + CBQ + 2 * GS;
-    static constexpr int FIXED = (even_up(EPK) + even_up(NPB)) / 2;    // packed product words (doubles)
+    static constexpr int QTOT0 = PERQ + CBQ + 2 * GS;
+    static constexpr int FIXED = even_up((even_up(EPK) + even_up(NPB)) / 2);   // packed product words (doubles)
+    // Bra product list of the bra primitive being drained, staged in shared memory: as many entries per quartet as the
+    // shared memory left over at the class's quartet count allows (the rest of the list is read from the L2 scratch).
+    static constexpr int SMEM_D = 232448 / 8;                  // 227 KB per CTA on sm_100a, in doubles
+    static constexpr int NQCAP = (192 / NCH) / NPG < 64 ? (192 / NCH) / NPG : 64;   // fused2_inst.cu: consumer threads per chunk
+    static constexpr int NQ0 = (SMEM_D - FIXED) / QTOT0 < NQCAP ? (SMEM_D - FIXED) / QTOT0 : NQCAP;
+    static constexpr int EPBS_ROOM = NQ0 < 1 ? 0 : (((SMEM_D - FIXED) / NQ0 - QTOT0) & ~1);
+    static constexpr int EPBS = EPBS_ROOM < 16 ? 0 : (EPBS_ROOM < even_up(NPB) ? EPBS_ROOM : even_up(NPB));
+    static constexpr int QTOT = QTOT0 + EPBS;
     static __host__ __device__ constexpr size_t smem_bytes(int nq) { return 8 * ((size_t)nq * QTOT + FIXED); }
 };
 

@@ -158,6 +158,7 @@ __global__ void __launch_bounds__(MD_F2_PRODUCERS + 192, 1) fused2_kernel(Fused2
     double *gsc = bufs + (size_t)NQ * C::CBQ;
     unsigned *packq = (unsigned *)(gsc + (size_t)2 * NQ * C::GS);          // [EPK]  ket product words
     unsigned *packc = packq + even_up(C::EPK);                             // [NPB]  bra product words
+    double *epb = gsc + (size_t)2 * NQ * C::GS + C::FIXED;                 // [NQ][EPBS] head of the bra product list being drained
     constexpr int O_OB = 2;
     constexpr int EPKe = even_up(C::EPK), NPBe = even_up(C::NPB);
     constexpr int KREC = 8 + EPKe, BRECS = 8 + NPBe;                       // scratch records: header + product list
@@ -270,30 +271,30 @@ __global__ void __launch_bounds__(MD_F2_PRODUCERS + 192, 1) fused2_kernel(Fused2
                 double oacc[C::NAB_C];
 #pragma unroll
                 for (int i = 0; i < C::NAB_C; ++i) oacc[i] = 0.0;
-                const double2 *ep = (const double2 *)(scr_bra(j, kb) + 8);     // bra product list, L2 scratch through L1
+                const double2 *ep = (const double2 *)(scr_bra(j, kb) + 8);     // tail of the bra product list: L2 scratch through L1
+                const double2 *es = (const double2 *)(epb + (size_t)j * C::EPBS);   // its head: staged by the consumers
                 constexpr ProdList<LA, LB, 0> PBL{};
                 double2 e2 = make_double2(0.0, 0.0);
                 static_for<PBL.N>([&](auto ic) {
                     constexpr int i = decltype(ic)::value;
-                    if constexpr ((i & 1) == 0) e2 = ep[i / 2];
+                    if constexpr ((i & 1) == 0) e2 = i < C::EPBS ? es[i / 2] : ep[i / 2];
                     oacc[PBL.comp[i]] = fma((i & 1) ? e2.y : e2.x, hv[PBL.off[i]], oacc[PBL.comp[i]]);
                 });
                 double o2[C::NAB_O];
                 solid2<LA, LB, PURE>(oacc, o2);
                 double *o = g.out + *(const long long *)(perq + (size_t)j * C::PERQ + O_OB) + (icd / C::NDO) * g.sc + (icd % C::NDO) * g.sd;
-                if (kb > 0) {                                // all loads first: the compiler cannot prove the elements distinct
-                    double prev[C::NAB_O];
+                if (kb > 0) {                                // later bra primitives: reduction in L2, nothing comes back
 #pragma unroll
                     for (int a = 0; a < C::NAO; ++a)
 #pragma unroll
-                        for (int b = 0; b < C::NBO; ++b) prev[a * C::NBO + b] = __ldcg(o + a * g.sa + b * g.sb);
+                        for (int b = 0; b < C::NBO; ++b)
+                            asm volatile("red.global.add.f64 [%0], %1;" ::"l"(o + a * g.sa + b * g.sb), "d"(o2[a * C::NBO + b]) : "memory");
+                } else {
 #pragma unroll
-                    for (int i = 0; i < C::NAB_O; ++i) o2[i] += prev[i];
+                    for (int a = 0; a < C::NAO; ++a)
+#pragma unroll
+                        for (int b = 0; b < C::NBO; ++b) o[a * g.sa + b * g.sb] = o2[a * C::NBO + b];
                 }
-#pragma unroll
-                for (int a = 0; a < C::NAO; ++a)
-#pragma unroll
-                    for (int b = 0; b < C::NBO; ++b) o[a * g.sa + b * g.sb] = o2[a * C::NBO + b];
             }
             bar_sync(DB, DN);                                // the drain region is free again
         };
@@ -301,6 +302,15 @@ __global__ void __launch_bounds__(MD_F2_PRODUCERS + 192, 1) fused2_kernel(Fused2
         if (consumer) {
             // ---------------- consumers: P4 over the ket primitives, then the drain ----------------
             for (int kb = 0; kb < Kbra; ++kb) {
+                // the previous drain is over for every participant: stage this primitive's bra product list behind P4
+                if constexpr (C::EPBS > 0) {
+                    constexpr int H = C::EPBS / 2;
+                    for (int c = tid; c < nqg * H; c += NC) {
+                        const int j = c / H, i = c - j * H;
+                        __pipeline_memcpy_async(epb + (size_t)j * C::EPBS + 2 * i, scr_bra(j, kb) + 8 + 2 * i, 16);
+                    }
+                    __pipeline_commit();
+                }
                 double hacc[PB][C::NACC];
 #pragma unroll
                 for (int k = 0; k < PB; ++k)
@@ -320,6 +330,7 @@ __global__ void __launch_bounds__(MD_F2_PRODUCERS + 192, 1) fused2_kernel(Fused2
                     if (b + 4 < B && !deferred(b)) bar_arrive(F2_BAR_EMPTY + buf, NC + NG);
                 }
                 const int dg = (kb * Kket + Kket - 1) & 1;
+                __pipeline_wait_prior(0);                    // this thread's part of the staged list has landed
                 bar_sync(F2_BAR_CONS, NC);                   // every consumer is done with group dg's buffers
                 if (cact && cj < nqg && ch == 0)
                     f2_flush<C, LC, LD, PURE, PB, false>(hacc, 0, ip, cbuf(2 * dg, cj) + C::O_HALF);
@@ -360,11 +371,11 @@ __global__ void __launch_bounds__(MD_F2_PRODUCERS + 192, 1) fused2_kernel(Fused2
                 }
                 bar_sync(F2_BAR_PROD + pgp, NG);
                 for (int it = gt; it < C::NZ * nqg; it += NG) {           // stage x (sorted by line length)
-                    int c = it / nqg;
-                    const int j = it - c * nqg;
-                    int s = 0;
-                    while (c > s) { c -= s + 1; ++s; }                    // column c of the anti-diagonal u+v = s
-                    I::x_task(c, s - c, gs0 + (size_t)j * C::GS, cbuf(buf, j));
+                    const int c = it / nqg, j = it - c * nqg;
+                    // column u of the anti-diagonal u + v = s: s = floor((sqrt(8c + 1) - 1)/2), exact in float for c < 2^20
+                    const int s = (int)((sqrtf((float)(8 * c + 1)) - 1.0f) * 0.5f);
+                    const int u = c - ((s * (s + 1)) >> 1);
+                    I::x_task(u, s - u, gs0 + (size_t)j * C::GS, cbuf(buf, j));
                 }
                 __pipeline_wait_prior(0);
                 bar_arrive(F2_BAR_FULL + buf, NC + NG);
