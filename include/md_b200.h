@@ -168,6 +168,22 @@ int md_exchange(const md_pairs *bra, const md_pairs *ket, int64_t nquartets, con
                 const int32_t *off_a, const int32_t *off_b, const int32_t *off_c, const int32_t *off_d, int64_t nao,
                 const double *D, double *K, void *cuda_stream);
 
+/*
+ * First geometric derivatives of (ab|cd): d/dR_i (ab|cd), R the centre of shell
+ * `center` (0, 1, 2, 3 = a, b, c, d), i = x, y, z.  By d/dA_i G_a = 2 zeta G_{a+1_i} - a_i G_{a-1_i} (Eq. 1) the
+ * derivative is the Cartesian integral with that shell raised (coefficients 2 zeta_k c_k) minus a_i times the one with
+ * it lowered; both come from the integral kernels, the combination and the solid-harmonic transform (Eq. 16) from
+ * kernels of their own.  The derivative with respect to the fourth centre follows from the other three (they sum to zero).
+ *   bra / ket / quartet_idx / pure / cuda_stream as for md_eri4 (4-center only); the differentiated shell needs
+ *   l <= MD_MAX_L - 1 (MD_EINVAL otherwise).
+ *   out (DEVICE): [q][i][a][b][c][d], 3 N_ab N_cd doubles per quartet, components as md_eri4 (MD_LAYOUT_QUARTET_MAJOR
+ *   only); out_capacity_elems is checked against 3 N_ab N_cd nquartets (MD_ECAPACITY).
+ * Scratch (the two Cartesian batches of a chunk of quartets, 64 MiB at most) comes from the stream-ordered pool.
+ * Asynchronous on cuda_stream.
+ */
+int md_eri4_grad(const md_pairs *bra, const md_pairs *ket, int64_t nquartets, const int32_t *quartet_idx, int pure,
+                 int center, double *out, int64_t out_capacity_elems, void *cuda_stream);
+
 /* Number of doubles the result occupies (negative error code on bad arguments). */
 int64_t md_eri4_out_elems(int la, int lb, int lc, int ld, int pure, int64_t nquartets);
 int64_t md_eri3_out_elems(int la, int lb, int lX, int pure, int64_t ntriplets);

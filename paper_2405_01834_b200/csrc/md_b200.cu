@@ -542,6 +542,146 @@ int run_exchange(const md_pairs *bra, const md_pairs *ket, long long nq, const i
     return e;
 }
 
+// ---- first geometric derivatives ----------------------------------------------------
+// A primitive Cartesian Gaussian (Eq. 1) depends on its centre A only through r - A:
+//     d/dA_i G_a = 2 zeta G_{a+1_i} - a_i G_{a-1_i}.
+// The derivative of (ab|cd) with respect to the centre of one shell is therefore the Cartesian integral batch with that
+// shell RAISED (l + 1, coefficients 2 zeta_k c_k) minus a_i times the batch with the shell LOWERED (l - 1).  Both batches come
+// from the integral kernels above (whatever variant the class selects); the kernels below form the coefficients, combine
+// the two batches component by component, and apply the solid-harmonic transform (Eq. 16, linear and centre-independent)
+// to the four indices afterwards.  A chunk of quartets at a time, so that the intermediates stay L2-sized.
+__global__ void grad_coefs_kernel(const double *exps, const double *coefs, double *out, long long n) {
+    const long long i = blockIdx.x * (long long)blockDim.x + threadIdx.x;
+    if (i < n) out[i] = 2.0 * exps[i] * coefs[i];
+}
+// position of the Cartesian component with exponents (., ay, az) inside its shell (include/md_b200.h: ax descending, then ay)
+__device__ __forceinline__ int grad_cart_pos(int ay, int az) { const int i = ay + az; return ((i * (i + 1)) >> 1) + az; }
+
+// G[q][i][pre][k][post] = U[q][pre][k + 1_i][post] - k_i Dn[q][pre][k - 1_i][post]; k runs over the Cartesian components of
+// the differentiated shell (angular momentum l), pre / post over the components of the shells before / after it.
+__global__ void grad_combine_kernel(const double *__restrict__ U, const double *__restrict__ Dn, double *__restrict__ G,
+                                    long long nq, int l, int pre, int post) {
+    const int nk = ncart(l), nu = ncart(l + 1), nd = l > 0 ? ncart(l - 1) : 0;
+    const long long per = (long long)pre * nk * post, total = nq * 3 * per;
+    for (long long t = blockIdx.x * (long long)blockDim.x + threadIdx.x; t < total; t += (long long)gridDim.x * blockDim.x) {
+        const long long q = t / (3 * per);
+        long long r = t - q * 3 * per;
+        const int i = (int)(r / per);
+        r -= (long long)i * per;
+        const int a = (int)(r / ((long long)nk * post));
+        r -= (long long)a * nk * post;
+        const int k = (int)(r / post), c = (int)(r - (long long)k * post);
+        int s = 0;                                       // k = s(s+1)/2 + az with s = ay + az
+        while (((s + 1) * (s + 2)) >> 1 <= k) ++s;
+        const int az = k - ((s * (s + 1)) >> 1), ay = s - az, ax = l - s;
+        const int ei = i == 0 ? ax : i == 1 ? ay : az;
+        const int ku = grad_cart_pos(ay + (i == 1), az + (i == 2));
+        double v = U[((q * pre + a) * nu + ku) * post + c];
+        if (ei > 0) {
+            const int kd = grad_cart_pos(ay - (i == 1), az - (i == 2));
+            v = fma(-(double)ei, Dn[((q * pre + a) * nd + kd) * post + c], v);
+        }
+        G[t] = v;
+    }
+}
+// One index of [outer][ncart(l)][inner] -> [outer][2l+1][inner] by the Cartesian->solid matrix of shell l (Eq. 16).
+__global__ void __launch_bounds__(256) grad_solid_kernel(const double *__restrict__ in, double *__restrict__ out, long long outer,
+                                                         int l, long long inner) {
+    __shared__ double C[13 * 28];
+    const int nin = ncart(l), nout = nsolid(l);
+    for (int i = threadIdx.x; i < nin * nout; i += blockDim.x) C[i] = c_solid[solid_off(l) + i];
+    __syncthreads();
+    const long long total = outer * nout * inner;
+    for (long long t = blockIdx.x * (long long)blockDim.x + threadIdx.x; t < total; t += (long long)gridDim.x * blockDim.x) {
+        const long long o = t / (nout * inner);
+        const long long r = t - o * nout * inner;
+        const int m = (int)(r / inner);
+        const long long c = r - m * inner;
+        const double *src = in + o * nin * inner + c;
+        double s = 0.0;
+        for (int k = 0; k < nin; ++k) s = fma(C[m * nin + k], src[k * inner], s);
+        out[t] = s;
+    }
+}
+
+int run_grad(const md_pairs *bra, const md_pairs *ket, long long nq, const int32_t *qidx, int pure, int center, double *out,
+             long long cap, cudaStream_t st) {
+    if (center < 0 || center > 3 || (pure != 0 && pure != 1) || nq < 0) return MD_EINVAL;
+    const md_shells *sh[4] = {&bra->a, &bra->b, &ket->a, &ket->b};
+    const int l = sh[center]->l;
+    if (l + 1 > MD_MAX_L) return MD_EINVAL;                       // the raised shell must be one the kernels serve
+    if (!qidx && nq != bra->npairs * ket->npairs) return MD_EINVAL;
+    long long pc = 1, po = 1;                                     // Cartesian / output components of one quartet block
+    for (int s = 0; s < 4; ++s) { pc *= ncart(sh[s]->l); po *= ncomp(sh[s]->l, pure); }
+    if (3 * po * nq > cap) return MD_ECAPACITY;
+    if (nq > 0 && !out) return MD_EINVAL;
+    int e = md_init();
+    if (e) return e;
+    S.last_launches = 0;
+    if (nq == 0) return MD_OK;
+    int pre = 1, post = 1;
+    for (int s = 0; s < center; ++s) pre *= ncart(sh[s]->l);
+    for (int s = center + 1; s < 4; ++s) post *= ncart(sh[s]->l);
+    const long long perU = pc / ncart(l) * ncart(l + 1), perD = l > 0 ? pc / ncart(l) * ncart(l - 1) : 0, perG = 3 * pc;
+    // raised and lowered shell batches: same centres and exponents
+    md_pairs up[2] = {*bra, *ket}, dn[2] = {*bra, *ket};
+    md_shells *su = center < 2 ? (center == 0 ? &up[0].a : &up[0].b) : (center == 2 ? &up[1].a : &up[1].b);
+    md_shells *sd = center < 2 ? (center == 0 ? &dn[0].a : &dn[0].b) : (center == 2 ? &dn[1].a : &dn[1].b);
+    const long long ncoef = (long long)sh[center]->n * sh[center]->K;
+    size_t budget = (size_t)64 << 20;
+    if (const char *env = getenv("MD_GRAD_CHUNK_BYTES")) budget = (size_t)atoll(env);
+    const size_t per_bytes = 8 * (size_t)(perU + perD + (pure ? 2 : 0) * perG);
+    const long long chunk = std::max<long long>(1, std::min<long long>(nq, (long long)(budget / std::max<size_t>(per_bytes, 1))));
+    double *coefs2 = nullptr, *U = nullptr, *Dn = nullptr, *G0 = nullptr, *G1 = nullptr;
+    int32_t *ci = nullptr;
+    CK(cudaMallocAsync(&coefs2, (size_t)std::max<long long>(ncoef, 1) * 8, st));
+    CK(cudaMallocAsync(&U, (size_t)chunk * (perU + perD) * 8, st));
+    Dn = U + chunk * perU;
+    if (pure) { CK(cudaMallocAsync(&G0, (size_t)chunk * perG * 16, st)); G1 = G0 + chunk * perG; }
+    if (!qidx) CK(cudaMallocAsync(&ci, (size_t)chunk * 2 * sizeof(int32_t), st));
+    int launches = 0;
+    if (ncoef > 0) { grad_coefs_kernel<<<(unsigned)((ncoef + 255) / 256), 256, 0, st>>>(sh[center]->exps, sh[center]->coefs, coefs2, ncoef); ++launches; }
+    su->l = l + 1; su->coefs = coefs2;
+    sd->l = l - 1;
+    const int ls[4] = {sh[0]->l, sh[1]->l, sh[2]->l, sh[3]->l};
+    for (long long q0 = 0; q0 < nq && e == MD_OK; q0 += chunk) {
+        const long long m = std::min(chunk, nq - q0);
+        const int32_t *qi = qidx ? qidx + 2 * q0 : ci;
+        if (!qidx) { product_idx_kernel<<<(unsigned)((m + 255) / 256), 256, 0, st>>>(ci, q0, m, ket->npairs); ++launches; }
+        e = run_call(view(up[0]), view(up[1]), m, qi, 0, MD_LAYOUT_QUARTET_MAJOR, U, m * perU, st);
+        launches += S.last_launches;
+        if (e == MD_OK && l > 0) {
+            e = run_call(view(dn[0]), view(dn[1]), m, qi, 0, MD_LAYOUT_QUARTET_MAJOR, Dn, m * perD, st);
+            launches += S.last_launches;
+        }
+        if (e != MD_OK) break;
+        const unsigned grid = (unsigned)std::min<long long>((m * perG + 255) / 256, (long long)S.nsm * 32);
+        double *dst = out + q0 * 3 * po;
+        grad_combine_kernel<<<grid, 256, 0, st>>>(U, Dn, pure ? G0 : dst, m, l, pre, post);
+        ++launches;
+        if (pure) {                                               // d, c, b, a in turn; the last pass writes the result
+            long long outer = m * 3 * (long long)ncart(ls[0]) * ncart(ls[1]) * ncart(ls[2]), inner = 1;
+            double *src = G0, *tmp = G1;
+            for (int s = 3; s >= 0; --s) {
+                double *to = s == 0 ? dst : tmp;
+                const long long total = outer * nsolid(ls[s]) * inner;
+                grad_solid_kernel<<<(unsigned)std::min<long long>((total + 255) / 256, (long long)S.nsm * 32), 256, 0, st>>>(src, to, outer, ls[s], inner);
+                ++launches;
+                inner *= nsolid(ls[s]);
+                if (s > 0) outer /= ncart(ls[s - 1]);
+                tmp = src; src = to;
+            }
+        }
+    }
+    if (ci) cudaFreeAsync(ci, st);
+    if (G0) cudaFreeAsync(G0, st);
+    cudaFreeAsync(U, st);
+    cudaFreeAsync(coefs2, st);
+    S.last_launches = launches;
+    if (e == MD_OK) CK(cudaGetLastError());
+    return e;
+}
+
 }  // namespace
 
 extern "C" {
@@ -643,6 +783,14 @@ int md_eri3(const md_pairs *bra, const md_shells *X, int64_t ntriplets, const in
     if ((e = check_shells(X))) return e;
     return run_call(view(*bra), view_single(*X), ntriplets, triplet_idx, pure, layout, out, out_capacity_elems,
                     (cudaStream_t)cuda_stream);
+}
+
+int md_eri4_grad(const md_pairs *bra, const md_pairs *ket, int64_t nquartets, const int32_t *quartet_idx, int pure,
+                 int center, double *out, int64_t out_capacity_elems, void *cuda_stream) {
+    int e = check_pairs(bra);
+    if (e) return e;
+    if ((e = check_pairs(ket))) return e;
+    return run_grad(bra, ket, nquartets, quartet_idx, pure, center, out, out_capacity_elems, (cudaStream_t)cuda_stream);
 }
 
 int md_exchange(const md_pairs *bra, const md_pairs *ket, int64_t nquartets, const int32_t *quartet_idx, int pure,
