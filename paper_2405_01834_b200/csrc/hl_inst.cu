@@ -93,7 +93,7 @@ bool make_plan(const HlCall &c0, int nsm, HlPlan &P) {
     const int ntile = (nnt_total + 3) / 4;
     int NW = (nnt_total + ntile - 1) / ntile;
     int warps, MW;
-    // By measurement (profiles/r02_hl_tune.md): 4-warp CTAs (three per SM) for the small classes, else 8 warps; the row tiles
+    // By measurement (profiles/r02_autotune.csv, hl rows): 4-warp CTAs (three per SM) for the small classes, else 8 warps; the row tiles
     // per warp that give the fewest tile slots over all row passes, weighted towards larger tiles (fewer gathers per DMMA).
     warps = (nmt <= 12 && nmt2 <= 4 * MD_HL_MT2) ? 4 : 8;
     MW = 1;

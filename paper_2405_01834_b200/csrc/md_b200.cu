@@ -356,7 +356,7 @@ int run_rules(const PairView &b, const PairView &k, long long nq, const int32_t 
                                b.a.l + (b.single ? 0 : b.b.l) >= 4 && nq >= 8 * (b.npairs + k.npairs);
     if (product_s_ket) return run_generic(b, k, nq, qidx, pure, layout, out, st, true, sc);
     // Every l <= 1, quartet-major output: one thread per quartet, registers only, coalesced tile stores (lowl.cuh).  By
-    // measurement (profiles/r02_lowl.md) it wins while the primitive loop is short; long contractions stay with the fused kernels.
+    // measurement (profiles/r02_autotune.csv) it wins while the primitive loop is short; long contractions stay with the fused kernels.
     if ((S.variant == MD_VARIANT_LOWL || (S.variant == MD_VARIANT_AUTO && (long long)s.Ka * s.Kb * s.Kc * s.Kd <= MD_LOWL_KMAX)) &&
         layout == MD_LAYOUT_QUARTET_MAJOR && lowl_has_class(b, k)) {
         if (sc.dry) { sc.need = 0; return MD_DRY; }
@@ -380,7 +380,7 @@ int run_rules(const PairView &b, const PairView &k, long long nq, const int32_t 
         }
     }
     if (S.variant == MD_VARIANT_AUTO || S.variant == MD_VARIANT_FUSED2) {
-        // By measurement (profiles/r01_sweep_l2.md): the warp-specialised kernel wins on every instantiated class
+        // By measurement (profiles/r01_sweep_l2.md, r02_autotune.csv): the warp-specialised kernel wins on every instantiated class
         // once the primitive loop is long enough to fill its pipeline, and on (dd|dd) for any K.
         const long long nprim = (long long)b.a.K * (b.single ? 1 : b.b.K) * k.a.K * (k.single ? 1 : k.b.K);
         const bool dddd = b.a.l == 2 && !b.single && b.b.l == 2 && k.a.l == 2 && !k.single && k.b.l == 2;
@@ -415,7 +415,7 @@ int run_rules(const PairView &b, const PairView &k, long long nq, const int32_t 
         out_strides(layout, qidx != nullptr, b.npairs, k.npairs, s.nab, s.ncd, c.s_q, c.s_bi, c.s_ki, c.s_ab, c.s_cd);
         c.boys_tab = S.boys_tab; c.rlut = fused_rlut();
         size_t need = 0;
-        // By measurement (profiles/r02_hl_tune.md): the one-launch kernel wins from (gg|gg) upward (N~_bra N~_ket >= 16,000:
+        // By measurement (profiles/r02_autotune.csv): the one-launch kernel wins from (gg|gg) upward (N~_bra N~_ket >= 16,000:
         // (gg|gg) 27,225, (fg|hi) 43,680); below that ((ff|ff) 7,056, (ff|i) 7,056) its per-quartet phases are too short
         // to fill a CTA and pair setup + the runtime-l kernels are faster.
         const bool large = (long long)s.nhb * s.nhk >= 16000;
