@@ -30,6 +30,10 @@ struct Eri3sArgs {
     int o_r0, o_r1, o_g, o_acc, o_e, o_ex, o_g0;   // offsets inside a warp's slice
 };
 
+// NXC = components of X in the result (2 lX + 1, or the Cartesian count), a compile-time constant so that the two hot loops
+// (Hobson G build, bra box loop) unroll exactly: with a run-time count every multiply-add carried a compare and its own
+// 8-byte shared-memory load (34 % + 28 % of the stall samples of (ff|f) K = 4, profiles/r02_eri3s.md).
+template <int NXC, bool PURE>
 __global__ void __launch_bounds__(256) eri3s_kernel(Eri3sArgs g) {
     extern __shared__ double sm[];
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
@@ -55,7 +59,8 @@ __global__ void __launch_bounds__(256) eri3s_kernel(Eri3sArgs g) {
     double *R0 = W + g.o_r0, *R1 = W + g.o_r1, *G = W + g.o_g, *acc = W + g.o_acc, *E = W + g.o_e, *EX = W + g.o_ex, *G0 = W + g.o_g0;
     const uint2 *lut = (const uint2 *)g.rlut;
     const int la = g.la, lb = g.lb, lX = g.lX, Lb = la + lb, L = g.L, nt = Lb + 1;
-    const int nca = g.nca, ncb = g.ncb, nXc = g.nXc, nhb = g.nhb, nab_c = nca * ncb;
+    constexpr int nXc = NXC;
+    const int nca = g.nca, ncb = g.ncb, nhb = g.nhb, nab_c = nca * ncb;
     const int esz = (la + 1) * (lb + 1) * nt;
     const uint32_t *ca = s_herm + nherm(la - 1), *cb = s_herm + nherm(lb - 1), *cx = s_herm + nherm(lX - 1);
     const int ncx = ncart(lX), nlow = nherm(lX - 1);
@@ -95,7 +100,7 @@ __global__ void __launch_bounds__(256) eri3s_kernel(Eri3sArgs g) {
                     G0[lane] = f;
                     if (lane == L) ((L & 1) ? R1 : R0)[0] = f;
                 }
-                if (!g.pure) hl_e_axis_warp(lX, 0, zx, 0.0, 0.0, EX, lane);   // one-centre table (Eq. 8), the same on the three axes
+                if (!PURE) hl_e_axis_warp(lX, 0, zx, 0.0, 0.0, EX, lane);   // one-centre table (Eq. 8), the same on the three axes
                 __syncwarp();
                 for (int m = L - 1; m >= 0; --m) {                   // Eq. 24, level m from level m + 1
                     const int ne = nherm(L - m);
@@ -115,25 +120,28 @@ __global__ void __launch_bounds__(256) eri3s_kernel(Eri3sArgs g) {
                     __syncwarp();
                 }
                 // G[p~][c] += sum_q~ H_X[q~][c] (-1)^{|q~|} [p~+q~]^(0)
-                if (g.pure) {
+                if constexpr (PURE) {
                     double f = (lX & 1) ? -1.0 : 1.0;                // Hobson: C^l_{m,q~}/(2 zeta)^l on the order-lX Hermites only
                     for (int i = 0; i < lX; ++i) f *= 0.5 / zx;
                     for (int ip = lane; ip < nhb; ip += 32) {          // lane = p~: 13 accumulators, C^{lX}[q~][m] broadcast to the warp
                         const uint32_t wp = s_herm[ip];
-                        double sacc[13];
+                        constexpr int NP = (nXc + 1) / 2;             // coefficient rows are zero-padded to MD_HL_CSTR: 16-byte loads
+                        double sacc[2 * NP];
 #pragma unroll
-                        for (int m = 0; m < 13; ++m) sacc[m] = 0.0;
+                        for (int m = 0; m < 2 * NP; ++m) sacc[m] = 0.0;
                         for (int j = 0; j < ncx; ++j) {
                             const double r = R0[hl_herm_index(wp + cx[j])];
-                            const double *c = CxT + j * MD_HL_CSTR;
+                            const double2 *c = (const double2 *)(CxT + j * MD_HL_CSTR);
 #pragma unroll
-                            for (int m = 0; m < 13; ++m)
-                                if (m < nXc) sacc[m] = fma(c[m], r, sacc[m]);
+                            for (int m = 0; m < NP; ++m) {
+                                const double2 cc = c[m];
+                                sacc[2 * m] = fma(cc.x, r, sacc[2 * m]);
+                                sacc[2 * m + 1] = fma(cc.y, r, sacc[2 * m + 1]);
+                            }
                         }
                         double *o = G + ip * nXc;
 #pragma unroll
-                        for (int m = 0; m < 13; ++m)
-                            if (m < nXc) o[m] = fma(f, sacc[m], o[m]);
+                        for (int m = 0; m < nXc; ++m) o[m] = fma(f, sacc[m], o[m]);
                     }
                 } else {
                     const int ntx = lX + 1;                          // EX[i*ntx + t]: E^t_i of the one-centre expansion
@@ -166,6 +174,7 @@ __global__ void __launch_bounds__(256) eri3s_kernel(Eri3sArgs g) {
                 unpack_tuv(ca[a], ax, ay, az);
                 unpack_tuv(cb[b], bx, by, bz);
                 const double *ex = Ex + (ax * (lb + 1) + bx) * nt, *ey = Ey + (ay * (lb + 1) + by) * nt, *ez = Ez + (az * (lb + 1) + bz) * nt;
+#pragma unroll
                 for (int c0 = 0; c0 < nXc; c0 += 7) {
                     double r[7];
 #pragma unroll
@@ -190,8 +199,8 @@ __global__ void __launch_bounds__(256) eri3s_kernel(Eri3sArgs g) {
             }
         }
         __syncwarp();
-        double *out = g.out + t * (long long)(g.pure ? nsolid(la) * nsolid(lb) : nab_c) * nXc;
-        if (!g.pure) {
+        double *out = g.out + t * (long long)(PURE ? nsolid(la) * nsolid(lb) : nab_c) * nXc;
+        if constexpr (!PURE) {
             for (int i = lane; i < nab_c * nXc; i += 32) out[i] = acc[i];
         } else {
             // Eq. 16 on a, then on b, through the R / G region (free now)

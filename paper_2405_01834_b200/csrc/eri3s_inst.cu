@@ -6,13 +6,34 @@
 
 namespace mdb {
 
-namespace { int g_e3_max_smem = 227 * 1024; }
+namespace {
+int g_e3_max_smem = 227 * 1024;
+typedef void (*E3Fn)(Eri3sArgs);
+E3Fn g_e3_fn[2][29];                          // [pure][number of X components in the result]
+
+template <int NXC, bool PURE>
+cudaError_t e3_reg(int max_smem) {
+    g_e3_fn[PURE][NXC] = eri3s_kernel<NXC, PURE>;
+    return cudaFuncSetAttribute(eri3s_kernel<NXC, PURE>, cudaFuncAttributeMaxDynamicSharedMemorySize, max_smem);
+}
+template <int LX>
+cudaError_t e3_reg_l(int max_smem) {
+    cudaError_t e = e3_reg<2 * LX + 1, true>(max_smem);
+    return e != cudaSuccess ? e : e3_reg<(LX + 1) * (LX + 2) / 2, false>(max_smem);
+}
+}  // namespace
 
 cudaError_t eri3s_init(int max_smem, const uint32_t *herm, const double *solid) {
     g_e3_max_smem = max_smem;
     cudaError_t e = upload_tables(herm, solid);
     if (e != cudaSuccess) return e;
-    return cudaFuncSetAttribute(eri3s_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, max_smem);
+    if ((e = e3_reg_l<0>(max_smem)) != cudaSuccess) return e;
+    if ((e = e3_reg_l<1>(max_smem)) != cudaSuccess) return e;
+    if ((e = e3_reg_l<2>(max_smem)) != cudaSuccess) return e;
+    if ((e = e3_reg_l<3>(max_smem)) != cudaSuccess) return e;
+    if ((e = e3_reg_l<4>(max_smem)) != cudaSuccess) return e;
+    if ((e = e3_reg_l<5>(max_smem)) != cudaSuccess) return e;
+    return e3_reg_l<6>(max_smem);
 }
 
 bool eri3s_has_class(const PairView &b, const PairView &k) {
@@ -49,7 +70,8 @@ int eri3s_dispatch(const PairView &b, const PairView &k, long long nt, const int
     const size_t smem = fixed + 8 * (size_t)o * warps;
     const int ctas = (int)std::max<size_t>(1, std::min<size_t>(2048 / threads, (size_t)(g_e3_max_smem + 1024) / (smem + 1024)));
     const long long nblk = (nt + warps - 1) / warps;
-    eri3s_kernel<<<(unsigned)std::min<long long>(nblk, (long long)nsm * ctas), threads, smem, st>>>(g);
+    if (!g_e3_fn[pure ? 1 : 0][g.nXc]) return 0;
+    g_e3_fn[pure ? 1 : 0][g.nXc]<<<(unsigned)std::min<long long>(nblk, (long long)nsm * ctas), threads, smem, st>>>(g);
     return 1;
 }
 
