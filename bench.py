@@ -490,7 +490,8 @@ def run_config5(args):
     t_schwarz = time.perf_counter() - t0
     vname = VARIANT_NAME
     rows = ["class,Kbra,Kket,pairs_bra,pairs_ket,quartets_passing,sampled,variant,ms,quartets_per_s,model_tflops,"
-            "extrapolated_s"]
+            "extrapolated_s" + (",measured_full_s,list_s" if args.full else "")]
+    full_s, list_s, full_q = 0.0, 0.0, 0
     rng = np.random.default_rng(5)
     tot_q, tot_s, tot_flop = 0, 0.0, 0.0
     name = lambda t: "spdfg"[t[0]] + (str(t[1]) if t[1] > 1 else "")
@@ -523,10 +524,38 @@ def run_config5(args):
             rate = len(qs) / (ms * 1e-3)
             fl = w.flops_model(True)
             cls = f"({name(pb[0])}{name(pb[1])}|{name(pk[0])}{name(pk[1])})"
-            rows.append(f"{cls},{pb[0][1] * pb[1][1]},{pk[0][1] * pk[1][1]},{len(pairs[pb])},{len(pairs[pk])},{count},{len(qs)},"
-                        f"{vname.get(engine.md_last_variant(), '?')},{ms:.4f},{rate:.4e},{fl * rate / 1e12:.3f},{count / rate:.3f}")
+            row = (f"{cls},{pb[0][1] * pb[1][1]},{pk[0][1] * pk[1][1]},{len(pairs[pb])},{len(pairs[pk])},{count},{len(qs)},"
+                   f"{vname.get(engine.md_last_variant(), '?')},{ms:.4f},{rate:.4e},{fl * rate / 1e12:.3f},{count / rate:.3f}")
             tot_q += count; tot_s += count / rate; tot_flop += fl * count
             del dw, out, dp, op
+            if args.full and max(pb[0][0], pb[1][0], pk[0][0], pk[1][0]) <= args.full_lmax:
+                # the class RUN IN FULL: the whole surviving list (built on the device), all pairs of both types, chunks of the
+                # list that reuse one output buffer (the integrals are not consumed: this times their evaluation)
+                t1 = time.perf_counter()
+                nfull, idx = engine.md_quartet_list(Qd[pb], Qd[pk], thr, same=same, capacity=count)
+                torch.cuda.synchronize()
+                tl = time.perf_counter() - t1
+                assert nfull == count
+                wf = W.config5_class(mol, pb, pk, pairs[pb], pairs[pk], np.zeros((1, 2), np.int32))
+                dwf = engine.DeviceWorkload(wf)
+                per = wf.nout(True)
+                chunk = int(max(1, min(count, (16 << 30) // (8 * per))))
+                outf = torch.empty(chunk * per, dtype=torch.float64, device="cuda")
+                e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+                e0.record()
+                for q0 in range(0, count, chunk):
+                    m = min(chunk, count - q0)
+                    engine.md_eri4(dwf.a, dwf.b, dwf.c, dwf.d, dwf.bra_idx, dwf.ket_idx, idx[q0:q0 + m], m, True, outf,
+                                   nbra=len(pairs[pb]), nket=len(pairs[pk]))
+                e1.record()
+                torch.cuda.synchronize()
+                tf = e0.elapsed_time(e1) * 1e-3
+                full_s += tf; list_s += tl; full_q += count
+                row += f",{tf:.4f},{tl:.4f}"
+                del idx, outf, dwf
+            elif args.full:
+                row += ",,"
+            rows.append(row)
     path = os.path.join(ROOT, "gpurun_out", "sweep_config5.csv")
     os.makedirs(os.path.dirname(path), exist_ok=True)
     open(path, "w").write("\n".join(rows) + "\n")
@@ -534,6 +563,8 @@ def run_config5(args):
                       "ao_solid": mol.nao(True), "shell_pairs": int(sum(len(p) for p in pairs.values())),
                       "schwarz_threshold": thr, "schwarz_seconds": t_schwarz, "quartets_passing": tot_q,
                       "extrapolated_sweep_seconds": tot_s, "extrapolated_model_tflops": tot_flop / tot_s / 1e12,
+                      **({"full_run": {"lmax": args.full_lmax, "quartets": full_q, "measured_seconds": full_s,
+                                       "list_seconds": list_s}} if args.full else {}),
                       "note": "per-class rate measured on a seeded sample of the surviving quartets; counts are exact"}))
 
 
@@ -581,6 +612,8 @@ def run_autotune(args):
                     cands = ["eri3s", "warp", "mma", "hl"] if lmax > 2 else ["eri3s", "fused", "fused2"]
                 else:
                     cands = ["warp", "mma", "hl"]
+                if not three and lmax >= 2 and ((ls[3] == 0 and max(ls[0], ls[1]) <= 3) or (ls[1] == 0 and max(ls[2], ls[3]) <= 3)):
+                    cands = cands + ["eri3s"]            # (ab|c s) / (a s|cd): the one-warp kernel with a two-centre ket
                 dw = engine.DeviceWorkload(w); out = dw.alloc_out(True)
                 best = None
                 seen = set()
@@ -688,6 +721,8 @@ def main():
     ap.add_argument("--variants", action="store_true", help="also time K=1 and Cartesian output")
     ap.add_argument("--cpu-sample", type=int, default=8000)
     ap.add_argument("--no-per-class", action="store_true", help="headline only (skip the per-class table)")
+    ap.add_argument("--full", action="store_true", help="--sweep config5: also RUN every class with all l <= --full-lmax in full")
+    ap.add_argument("--full-lmax", type=int, default=4)
     ap.add_argument("--case", default=None, help="run ONE per-class case once on --count-n quartets (for ncu instruction counts)")
     ap.add_argument("--count-n", type=int, default=2000)
     ap.add_argument("--variant", default=None, help="with --case: force this kernel variant (generic|fused|mma|fused2|warp|hl)")

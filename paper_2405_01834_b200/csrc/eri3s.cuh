@@ -18,7 +18,11 @@ namespace mdb {
 
 struct Eri3sArgs {
     PairView bra;
-    ShellView X;
+    ShellView X;                          // the one-centre ket shell, or shell c of a two-centre ket (c, s)
+    ShellView D;                          // two-centre ket: its s shell d
+    const int32_t *kidx;                  // two-centre ket: pair list (c, d) or nullptr
+    int KD, swap;                         // swap = 1: the kernel's bra is the CALLER's ket (index columns and output strides swapped)
+    long long s_t, s_ab, s_c;             // output strides (doubles) of the triplet / quartet, the ab block index, the c index
     int pure, la, lb, lX, Ka, Kb, KX;
     int nca, ncb, nXc, nhb, L;            // Cartesian counts of a, b; components of X in the result; N~(la+lb); la+lb+lX
     const int32_t *tidx;                  // [n][2] (bra pair, X shell) or nullptr: product, X fastest
@@ -33,8 +37,12 @@ struct Eri3sArgs {
 // NXC = components of X in the result (2 lX + 1, or the Cartesian count), a compile-time constant so that the two hot loops
 // (Hobson G build, bra box loop) unroll exactly: with a run-time count every multiply-add carried a compare and its own
 // 8-byte shared-memory load (34 % + 28 % of the stall samples of (ff|f) K = 4, profiles/r02_eri3s.md).
-template <int NXC, bool PURE>
+// MODE 0: one-centre solid X (Hobson form); 1: one-centre Cartesian X; 2: two-centre ket (c, s_d) of a 4-center class -- G is
+// built in the Cartesian components of c from the three 1-D tables of the pair (Eqs. 9, 10, 13: the s shell only moves the
+// centre and adds the exponential), and the solid transform of c (Eq. 16), if asked for, is a third pass at the end.
+template <int NXC, int MODE>
 __global__ void __launch_bounds__(256) eri3s_kernel(Eri3sArgs g) {
+    constexpr bool PURE = MODE == 0, TWO = MODE == 2;
     extern __shared__ double sm[];
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
     // CTA-wide constants: Hermite triples and the transposed Cartesian->solid tables of a, b, X
@@ -68,13 +76,20 @@ __global__ void __launch_bounds__(256) eri3s_kernel(Eri3sArgs g) {
 
     for (long long t = (long long)blockIdx.x * g.warps + warp; t < g.nt; t += wstride) {
         long long bi, xi;
-        if (g.tidx) { bi = g.tidx[2 * t]; xi = g.tidx[2 * t + 1]; }
-        else { bi = t / g.nX; xi = t % g.nX; }
-        long long ia = bi, ib = bi;
+        if (g.tidx) { bi = g.tidx[2 * t + g.swap]; xi = g.tidx[2 * t + 1 - g.swap]; }
+        else {
+            const long long b0 = t / g.nX, k0 = t % g.nX;            // the caller's (bra, ket) of product entry t
+            bi = g.swap ? k0 : b0; xi = g.swap ? b0 : k0;
+        }
+        long long ia = bi, ib = bi, id = xi;
         if (g.bra.idx) { ia = g.bra.idx[2 * bi]; ib = g.bra.idx[2 * bi + 1]; }
-        double A[3], B[3], Xc[3];
+        if (TWO && g.kidx) { id = g.kidx[2 * xi + 1]; xi = g.kidx[2 * xi]; }
+        double A[3], B[3], Xc[3], Dc[3];
 #pragma unroll
-        for (int x = 0; x < 3; ++x) { A[x] = g.bra.a.center[3 * ia + x]; B[x] = g.bra.b.center[3 * ib + x]; Xc[x] = g.X.center[3 * xi + x]; }
+        for (int x = 0; x < 3; ++x) {
+            A[x] = g.bra.a.center[3 * ia + x]; B[x] = g.bra.b.center[3 * ib + x]; Xc[x] = g.X.center[3 * xi + x];
+            Dc[x] = TWO ? g.D.center[3 * id + x] : Xc[x];
+        }
         for (int i = lane; i < nab_c * nXc; i += 32) acc[i] = 0.0;
         for (int kab = 0; kab < g.Ka * g.Kb; ++kab) {
             const int ka = kab / g.Kb, kb = kab - ka * g.Kb;
@@ -88,8 +103,18 @@ __global__ void __launch_bounds__(256) eri3s_kernel(Eri3sArgs g) {
             double PQ[3];
 #pragma unroll
             for (int x = 0; x < 3; ++x) PQ[x] = (za * A[x] + zb * B[x]) / p - Xc[x];
-            for (int kx = 0; kx < g.KX; ++kx) {
-                const double zx = g.X.exps[xi * g.KX + kx], cxc = g.X.coefs[xi * g.KX + kx];
+            for (int kx = 0; kx < g.KX * (TWO ? g.KD : 1); ++kx) {
+                double zx, cxc, zc = 0.0, zd = 0.0;                  // zx: the ket exponent q (one-centre: zeta_X)
+                if constexpr (TWO) {
+                    const int kc = kx / g.KD, kd = kx - kc * g.KD;
+                    zc = g.X.exps[xi * g.KX + kc]; zd = g.D.exps[id * g.KD + kd];
+                    cxc = g.X.coefs[xi * g.KX + kc] * g.D.coefs[id * g.KD + kd];
+                    zx = zc + zd;
+#pragma unroll
+                    for (int x = 0; x < 3; ++x) PQ[x] = (za * A[x] + zb * B[x]) / p - (zc * Xc[x] + zd * Dc[x]) / zx;
+                } else {
+                    zx = g.X.exps[xi * g.KX + kx]; cxc = g.X.coefs[xi * g.KX + kx];
+                }
                 const double rho = p * zx / (p + zx);
                 const double T = rho * (PQ[0] * PQ[0] + PQ[1] * PQ[1] + PQ[2] * PQ[2]);
                 __syncwarp();
@@ -100,7 +125,10 @@ __global__ void __launch_bounds__(256) eri3s_kernel(Eri3sArgs g) {
                     G0[lane] = f;
                     if (lane == L) ((L & 1) ? R1 : R0)[0] = f;
                 }
-                if (!PURE) hl_e_axis_warp(lX, 0, zx, 0.0, 0.0, EX, lane);   // one-centre table (Eq. 8), the same on the three axes
+                if constexpr (TWO) {                                 // the pair (c, s): E^t_{i0} per axis, exponential included (Eq. 13)
+#pragma unroll
+                    for (int x = 0; x < 3; ++x) hl_e_axis_warp(lX, 0, zc, zd, Xc[x] - Dc[x], EX + x * (lX + 1) * (lX + 1), lane);
+                } else if (!PURE) hl_e_axis_warp(lX, 0, zx, 0.0, 0.0, EX, lane);   // one-centre table (Eq. 8), the same on the three axes
                 __syncwarp();
                 for (int m = L - 1; m >= 0; --m) {                   // Eq. 24, level m from level m + 1
                     const int ne = nherm(L - m);
@@ -143,6 +171,48 @@ __global__ void __launch_bounds__(256) eri3s_kernel(Eri3sArgs g) {
 #pragma unroll
                         for (int m = 0; m < nXc; ++m) o[m] = fma(f, sacc[m], o[m]);
                     }
+                } else if constexpr (nXc <= 15) {
+                    // l_X <= 4: the dense table HX[q~][c] = (-1)^{|q~|} E^t_{cx} E^u_{cy} E^v_{cz} of this ket primitive (Eqs. 7, 8, 19;
+                    // zero where a Hermite index exceeds the Cartesian one), then lane = p~ with every column in registers: three
+                    // times the multiply-adds of the sparse walk below, but no per-element box loop and no divergence
+                    const int ntx = lX + 1, nhx = nherm(lX), exsz = (TWO ? 3 : 1) * ntx * ntx;
+                    const double *EY = TWO ? EX + ntx * ntx : EX, *EZ = TWO ? EX + 2 * ntx * ntx : EX;
+                    constexpr int NP = (nXc + 1) / 2, HS = 2 * NP;
+                    double *HX = EX + exsz + (exsz & 1);
+                    for (int i = lane; i < nhx * HS; i += 32) {
+                        const int iq = i / HS, c = i - iq * HS;
+                        double e3 = 0.0;
+                        if (c < nXc) {
+                            int ex, ey, ez, t2, u2, v2;
+                            unpack_tuv(cx[c], ex, ey, ez);
+                            unpack_tuv(s_herm[iq], t2, u2, v2);
+                            if (t2 <= ex && u2 <= ey && v2 <= ez) {
+                                e3 = EX[ex * ntx + t2] * EY[ey * ntx + u2] * EZ[ez * ntx + v2];
+                                if ((t2 + u2 + v2) & 1) e3 = -e3;
+                            }
+                        }
+                        HX[i] = e3;
+                    }
+                    __syncwarp();
+                    for (int ip = lane; ip < nhb; ip += 32) {
+                        const uint32_t wp = s_herm[ip];
+                        double sacc[HS];
+#pragma unroll
+                        for (int m = 0; m < HS; ++m) sacc[m] = 0.0;
+                        for (int iq = 0; iq < nhx; ++iq) {
+                            const double r = R0[hl_herm_index(wp + s_herm[iq])];
+                            const double2 *h = (const double2 *)(HX + iq * HS);
+#pragma unroll
+                            for (int m = 0; m < NP; ++m) {
+                                const double2 hh = h[m];
+                                sacc[2 * m] = fma(hh.x, r, sacc[2 * m]);
+                                sacc[2 * m + 1] = fma(hh.y, r, sacc[2 * m + 1]);
+                            }
+                        }
+                        double *o = G + ip * nXc;
+#pragma unroll
+                        for (int m = 0; m < nXc; ++m) o[m] += sacc[m];
+                    }
                 } else {
                     const int ntx = lX + 1;                          // EX[i*ntx + t]: E^t_i of the one-centre expansion
                     for (int i = lane; i < nhb * nXc; i += 32) {
@@ -151,10 +221,12 @@ __global__ void __launch_bounds__(256) eri3s_kernel(Eri3sArgs g) {
                         int ex, ey, ez;
                         unpack_tuv(cx[c], ex, ey, ez);
                         double s = 0.0;
-                        for (int t2 = ex & 1; t2 <= ex; t2 += 2)     // Eq. 12: E^t_i = 0 unless t = i mod 2
-                            for (int u2 = ey & 1; u2 <= ey; u2 += 2)
-                                for (int v2 = ez & 1; v2 <= ez; v2 += 2) {
-                                    const double e3 = EX[ex * ntx + t2] * EX[ey * ntx + u2] * EX[ez * ntx + v2];
+                        constexpr int st = TWO ? 1 : 2;              // Eq. 12 (one centre): E^t_i = 0 unless t = i mod 2
+                        const double *EY = TWO ? EX + ntx * ntx : EX, *EZ = TWO ? EX + 2 * ntx * ntx : EX;
+                        for (int t2 = TWO ? 0 : ex & 1; t2 <= ex; t2 += st)
+                            for (int u2 = TWO ? 0 : ey & 1; u2 <= ey; u2 += st)
+                                for (int v2 = TWO ? 0 : ez & 1; v2 <= ez; v2 += st) {
+                                    const double e3 = EX[ex * ntx + t2] * EY[ey * ntx + u2] * EZ[ez * ntx + v2];
                                     const uint32_t wq = (uint32_t)t2 | (uint32_t)u2 << 8 | (uint32_t)v2 << 16 | (uint32_t)(t2 + u2 + v2) << 24;
                                     const double r = R0[hl_herm_index(wp + wq)];
                                     s = ((t2 + u2 + v2) & 1) ? fma(-e3, r, s) : fma(e3, r, s);
@@ -199,9 +271,9 @@ __global__ void __launch_bounds__(256) eri3s_kernel(Eri3sArgs g) {
             }
         }
         __syncwarp();
-        double *out = g.out + t * (long long)(PURE ? nsolid(la) * nsolid(lb) : nab_c) * nXc;
-        if constexpr (!PURE) {
-            for (int i = lane; i < nab_c * nXc; i += 32) out[i] = acc[i];
+        double *out = g.out + t * g.s_t;
+        if (!PURE && !(TWO && g.pure)) {
+            for (int i = lane; i < nab_c * nXc; i += 32) { const int ab = i / nXc, c = i - ab * nXc; out[ab * g.s_ab + c * g.s_c] = acc[i]; }
         } else {
             // Eq. 16 on a, then on b, through the R / G region (free now)
             const int nsa = nsolid(la), nsb = nsolid(lb);
@@ -235,9 +307,26 @@ __global__ void __launch_bounds__(256) eri3s_kernel(Eri3sArgs g) {
                     for (int m = 0; m < 7; ++m)
                         if (m < nsb) oacc[m] = fma(cc[m], v, oacc[m]);
                 }
+                if constexpr (TWO) {                                 // c is still Cartesian: [ma mb][c] goes to the acc region (free now)
 #pragma unroll
-                for (int m = 0; m < 7; ++m)
-                    if (m < nsb) out[(ma * nsb + m) * nXc + c] = oacc[m];
+                    for (int m = 0; m < 7; ++m)
+                        if (m < nsb) acc[(ma * nsb + m) * nXc + c] = oacc[m];
+                } else {
+#pragma unroll
+                    for (int m = 0; m < 7; ++m)
+                        if (m < nsb) out[(ma * nsb + m) * g.s_ab + c * g.s_c] = oacc[m];
+                }
+            }
+            if constexpr (TWO) {                                     // Eq. 16 on c
+                __syncwarp();
+                const int nsx = nsolid(lX);
+                for (int i = lane; i < nsa * nsb * nsx; i += 32) {
+                    const int ab = i / nsx, m = i - ab * nsx;
+                    double v = 0.0;
+#pragma unroll
+                    for (int c = 0; c < nXc; ++c) v = fma(CxT[c * MD_HL_CSTR + m], acc[ab * nXc + c], v);
+                    out[ab * g.s_ab + m * g.s_c] = v;
+                }
             }
         }
         __syncwarp();

@@ -9,17 +9,19 @@ namespace mdb {
 namespace {
 int g_e3_max_smem = 227 * 1024;
 typedef void (*E3Fn)(Eri3sArgs);
-E3Fn g_e3_fn[2][29];                          // [pure][number of X components in the result]
+E3Fn g_e3_fn[3][29];                          // [mode][number of ket columns]: eri3s.cuh
 
-template <int NXC, bool PURE>
+template <int NXC, int MODE>
 cudaError_t e3_reg(int max_smem) {
-    g_e3_fn[PURE][NXC] = eri3s_kernel<NXC, PURE>;
-    return cudaFuncSetAttribute(eri3s_kernel<NXC, PURE>, cudaFuncAttributeMaxDynamicSharedMemorySize, max_smem);
+    g_e3_fn[MODE][NXC] = eri3s_kernel<NXC, MODE>;
+    return cudaFuncSetAttribute(eri3s_kernel<NXC, MODE>, cudaFuncAttributeMaxDynamicSharedMemorySize, max_smem);
 }
 template <int LX>
 cudaError_t e3_reg_l(int max_smem) {
-    cudaError_t e = e3_reg<2 * LX + 1, true>(max_smem);
-    return e != cudaSuccess ? e : e3_reg<(LX + 1) * (LX + 2) / 2, false>(max_smem);
+    cudaError_t e = e3_reg<2 * LX + 1, 0>(max_smem);
+    if (e != cudaSuccess) return e;
+    if ((e = e3_reg<(LX + 1) * (LX + 2) / 2, 1>(max_smem)) != cudaSuccess) return e;
+    return e3_reg<(LX + 1) * (LX + 2) / 2, 2>(max_smem);
 }
 }  // namespace
 
@@ -36,19 +38,29 @@ cudaError_t eri3s_init(int max_smem, const uint32_t *herm, const double *solid) 
     return e3_reg_l<6>(max_smem);
 }
 
+// 3-center (ab|X), or a 4-center class with an s shell second in one pair -- (ab|c s) or (a s|cd) -- whose other pair has l <= 3.
 bool eri3s_has_class(const PairView &b, const PairView &k) {
-    return k.single && !b.single && b.a.l <= 3 && b.b.l <= 3;
+    if (b.single) return false;
+    if (k.single) return b.a.l <= 3 && b.b.l <= 3;
+    return (k.b.l == 0 && b.a.l <= 3 && b.b.l <= 3) || (b.b.l == 0 && k.a.l <= 3 && k.b.l <= 3);
 }
 
-int eri3s_dispatch(const PairView &b, const PairView &k, long long nt, const int32_t *tidx, int pure, double *out,
+int eri3s_dispatch(const PairView &b0, const PairView &k0, long long nt, const int32_t *tidx, int pure, double *out,
                    const double *boys_tab, const uint32_t *rlut, int nsm, cudaStream_t st) {
-    if (!eri3s_has_class(b, k)) return 0;
+    if (!eri3s_has_class(b0, k0)) return 0;
+    const bool two = !k0.single;
+    const bool swap = two && !(k0.b.l == 0 && b0.a.l <= 3 && b0.b.l <= 3);      // the caller's bra is the pair with the s shell
+    const PairView &b = swap ? k0 : b0, &k = swap ? b0 : k0;
     Eri3sArgs g;
-    g.bra = b; g.X = k.a; g.pure = pure;
+    g.bra = b; g.X = k.a; g.D = k.b; g.kidx = two ? k.idx : nullptr; g.KD = two ? k.b.K : 1; g.swap = swap ? 1 : 0; g.pure = pure;
     g.la = b.a.l; g.lb = b.b.l; g.lX = k.a.l; g.Ka = b.a.K; g.Kb = b.b.K; g.KX = k.a.K;
-    g.nca = ncart(g.la); g.ncb = ncart(g.lb); g.nXc = ncomp(g.lX, pure);
+    g.nca = ncart(g.la); g.ncb = ncart(g.lb); g.nXc = two ? ncart(g.lX) : ncomp(g.lX, pure);
     g.nhb = nherm(g.la + g.lb); g.L = g.la + g.lb + g.lX;
-    g.tidx = tidx; g.nt = nt; g.nX = k.npairs; g.out = out; g.boys_tab = boys_tab; g.rlut = rlut;
+    g.tidx = tidx; g.nt = nt; g.nX = k0.npairs; g.out = out; g.boys_tab = boys_tab; g.rlut = rlut;
+    const long long nab_o = (long long)ncomp(g.la, pure) * ncomp(g.lb, pure), nc_o = ncomp(g.lX, pure);
+    g.s_t = nab_o * nc_o;
+    g.s_ab = swap ? 1 : nc_o;                                  // [a][b][c][d = s]; swapped: the kernel's c is the caller's a
+    g.s_c = swap ? nab_o : 1;
     auto even = [](int x) { return x + (x & 1); };
     int o = 0;
     g.o_r0 = o; o += even(nherm(g.L));
@@ -56,7 +68,8 @@ int eri3s_dispatch(const PairView &b, const PairView &k, long long nt, const int
     g.o_g = o; o += even(g.nhb * g.nXc);
     g.o_acc = o; o += even(g.nca * g.ncb * g.nXc);
     g.o_e = o; o += even(3 * (g.la + 1) * (g.lb + 1) * (g.la + g.lb + 1));
-    g.o_ex = o; o += even((g.lX + 1) * (g.lX + 1));
+    g.o_ex = o; o += even((two ? 3 : 1) * (g.lX + 1) * (g.lX + 1));
+    if ((two || !pure) && g.nXc <= 15) o += nherm(g.lX) * even(g.nXc);       // the dense table HX[q~][c] of one ket primitive
     g.o_g0 = o; o += even(g.L + 1);
     g.per_warp = o;
     const size_t fixed = 8 * (228 + 4 * 28 * MD_HL_CSTR + 88);   // Hermite triples, four transposed solid tables, the (t,u,v) cube
@@ -70,8 +83,9 @@ int eri3s_dispatch(const PairView &b, const PairView &k, long long nt, const int
     const size_t smem = fixed + 8 * (size_t)o * warps;
     const int ctas = (int)std::max<size_t>(1, std::min<size_t>(2048 / threads, (size_t)(g_e3_max_smem + 1024) / (smem + 1024)));
     const long long nblk = (nt + warps - 1) / warps;
-    if (!g_e3_fn[pure ? 1 : 0][g.nXc]) return 0;
-    g_e3_fn[pure ? 1 : 0][g.nXc]<<<(unsigned)std::min<long long>(nblk, (long long)nsm * ctas), threads, smem, st>>>(g);
+    const int mode = two ? 2 : pure ? 0 : 1;
+    if (!g_e3_fn[mode][g.nXc]) return 0;
+    g_e3_fn[mode][g.nXc]<<<(unsigned)std::min<long long>(nblk, (long long)nsm * ctas), threads, smem, st>>>(g);
     return 1;
 }
 

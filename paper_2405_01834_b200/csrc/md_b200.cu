@@ -369,7 +369,9 @@ int run_rules(const PairView &b, const PairView &k, long long nq, const int32_t 
     }
     // 3-center with la, lb <= 3 (BASELINE configs[2]): one warp per triplet in the sparse Cartesian form (eri3s.cuh); by
     // measurement (profiles/r02_eri3s.md) under AUTO for every such class that has an l >= 2 shell.
-    if ((S.variant == MD_VARIANT_ERI3S || (S.variant == MD_VARIANT_AUTO && std::max({s.la, s.lb, s.lc}) >= 2)) &&
+    // The same kernel serves 4-center classes with an s shell second in one pair, (ab|c s) or (a s|cd); those only when the
+    // table (or the caller) names it.
+    if ((S.variant == MD_VARIANT_ERI3S || (S.variant == MD_VARIANT_AUTO && k.single && std::max({s.la, s.lb, s.lc}) >= 2)) &&
         layout == MD_LAYOUT_QUARTET_MAJOR && eri3s_has_class(b, k)) {
         if (sc.dry) { sc.need = 0; return MD_DRY; }
         if (eri3s_dispatch(b, k, nq, qidx, pure, out, S.boys_tab, fused_rlut(), S.nsm, st) == 1) {
@@ -442,6 +444,10 @@ int run(const PairView &b, const PairView &k, long long nq, const int32_t *qidx,
     int tv = 0;
     if (!product_mode && layout == MD_LAYOUT_QUARTET_MAJOR && !b.single)
         tv = table_variant(s.la, s.lb, s.lc, s.ld, k.single != 0, (long long)s.Ka * s.Kb * s.Kc * s.Kd > 1);
+    // The table was measured on independent quartets, where every quartet pays its own pair setup.  The one-warp kernel's
+    // 4-center form recomputes its 1-D tables per quartet; when pairs are shared by many quartets (a screened molecule list) the
+    // kernels that read per-pair records win that case back (1.3e8 against about 5e7 quartets/s on (fd|ds)), so the rules decide.
+    if (tv == MD_VARIANT_ERI3S && !k.single && nq >= 8 * (b.npairs + k.npairs)) tv = 0;
     if (!tv) return run_rules(b, k, nq, qidx, pure, layout, out, cap, st, sc);
     S.variant = tv;
     int e = run_rules(b, k, nq, qidx, pure, layout, out, cap, st, sc);

@@ -97,9 +97,12 @@ __global__ void __launch_bounds__(MD_WARP_THREADS) eri_warp_kernel(WarpArgs g) {
                 // [p~+q~] feeds 8 FMAs and the Hk loads are warp-wide broadcasts; else one (p~, cd) element per lane.
                 const double *Hk = rk + 4;
                 if (nhb >= 16 && g.ncd >= 4) {
-                    for (int cd0 = 0; cd0 < g.ncd; cd0 += 8) {
-                        const int nc = min(8, g.ncd - cd0);
-                        for (int p = lane; p < nhb; p += 32) {
+                    // tasks (row p~, chunk of 8 columns) are dealt to the lanes together: 35 rows x 2 chunks take 3 rounds, not 4
+                    const int nchunk = (g.ncd + 7) >> 3;
+                    for (int task = lane; task < nhb * nchunk; task += 32) {
+                        {
+                            const int ch = task / nhb, p = task - ch * nhb, cd0 = ch << 3;
+                            const int nc = min(8, g.ncd - cd0);
                             const uint32_t wp = s_w[p];
                             double acc[8];
 #pragma unroll
@@ -131,10 +134,12 @@ __global__ void __launch_bounds__(MD_WARP_THREADS) eri_warp_kernel(WarpArgs g) {
             __syncwarp();
             // S4b: [ab|cd] (+)= sum_p~ Hb[p~][ab] [p~|cd]                    (Eq. 26); S5 is folded into Hb, Hk
             const double *Hb = rb + 4;
-            if (g.nab >= 16 && g.ncd >= 4) {                   // lanes own ab, 8 columns cd in registers
-                for (int cd0 = 0; cd0 < g.ncd; cd0 += 8) {
-                    const int nc = min(8, g.ncd - cd0);
-                    for (int ab = lane; ab < g.nab; ab += 32) {
+            if (g.nab >= 16 && g.ncd >= 4) {                   // a lane owns (ab, chunk of 8 columns cd) in registers
+                const int nchunk = (g.ncd + 7) >> 3;
+                for (int task = lane; task < g.nab * nchunk; task += 32) {
+                    {
+                        const int ch = task / g.nab, ab = task - ch * g.nab, cd0 = ch << 3;
+                        const int nc = min(8, g.ncd - cd0);
                         double acc[8];
 #pragma unroll
                         for (int c = 0; c < 8; ++c) acc[c] = 0.0;

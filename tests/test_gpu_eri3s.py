@@ -42,3 +42,36 @@ def test_eri3s_index_lists_and_product_mode():
         for pure in (True, False):
             _, used = check(w, pure, E3)
             assert used == E3
+
+
+# ---- the same kernel on 4-center classes with an s shell second in one pair: (ab|c s) and, by swapping sides, (a s|cd) ----
+
+TWO = [((3, 2, 2, 0), (1, 1, 1, 1)), ((2, 1, 4, 0), (2, 1, 1, 2)), ((3, 3, 6, 0), (1, 1, 1, 1)), ((1, 0, 0, 0), (1, 2, 2, 1)),
+       ((3, 3, 3, 0), (2, 2, 1, 3)), ((0, 0, 5, 0), (1, 1, 1, 1)),
+       ((3, 0, 2, 1), (1, 1, 1, 1)), ((5, 0, 3, 3), (1, 1, 1, 1)), ((4, 0, 1, 1), (2, 2, 1, 1)), ((6, 0, 3, 2), (1, 1, 2, 1))]
+
+
+@pytest.mark.parametrize("ls,Ks", TWO, ids=[str(c[0]) for c in TWO])
+def test_eri3s_two_centre_ket_with_an_s_shell(ls, Ks):
+    w = W.class_sweep(ls, 41, K=Ks)
+    for pure in (True, False):
+        _, used = check(w, pure, E3)
+        assert used == E3
+
+
+def test_eri3s_two_centre_index_lists_and_product_mode():
+    rng = np.random.default_rng(22)
+    a = W.make_shells(rng, 9, 3, 2, (0.2, 8.0), (-1.5, 1.5))
+    b = W.make_shells(rng, 7, 1, 1, (0.2, 8.0), (-1.5, 1.5))
+    c = W.make_shells(rng, 5, 4, 1, (0.2, 8.0), (-1.5, 1.5))
+    d = W.make_shells(rng, 6, 0, 2, (0.2, 8.0), (-1.5, 1.5))
+    bra_idx = np.stack([rng.integers(0, 9, 31), rng.integers(0, 7, 31)], 1).astype(np.int32)
+    ket_idx = np.stack([rng.integers(0, 5, 23), rng.integers(0, 6, 23)], 1).astype(np.int32)
+    qi = np.stack([rng.integers(0, 31, 120), rng.integers(0, 23, 120)], 1).astype(np.int32)
+    for q in (qi, None):
+        for pure in (True, False):
+            _, used = check(W.Workload("e3two", a, b, c, d, bra_idx, ket_idx, q), pure, E3)          # (fp|g s)
+            assert used == E3
+            _, used = check(W.Workload("e3swap", c, d, a, b, ket_idx, bra_idx,                        # (g s|fp): sides swapped
+                                       None if q is None else q[:, ::-1].copy()), pure, E3)
+            assert used == E3
