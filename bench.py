@@ -569,6 +569,18 @@ def run_config5(args):
 
 
 
+def e3_serves(ls):
+    """Mirror of eri3s_has_class for 4-center classes: one pair with both l <= 3, the other (c s) or small enough for the dense ket table."""
+    nc = lambda l: (l + 1) * (l + 2) // 2
+    nh = lambda l: (l + 1) * (l + 2) * (l + 3) // 6
+    bra_ok = lambda a, b: a <= 3 and b <= 3
+
+    def ket_ok(c, d):
+        ncol = nc(c) * nc(d)
+        return d == 0 or (ncol <= 36 and nh(c + d) * (ncol + ncol % 2) <= 1536)
+    return (bra_ok(ls[0], ls[1]) and ket_ok(ls[2], ls[3])) or (bra_ok(ls[2], ls[3]) and ket_ok(ls[0], ls[1]))
+
+
 def run_autotune(args):
     """Times every candidate kernel variant on every canonical class (K = 1; K = 2 per shell for classes with all l <= 3) in the
     independent-quartet structure and writes the measured-best table the library's AUTO consults:
@@ -612,8 +624,8 @@ def run_autotune(args):
                     cands = ["eri3s", "warp", "mma", "hl"] if lmax > 2 else ["eri3s", "fused", "fused2"]
                 else:
                     cands = ["warp", "mma", "hl"]
-                if not three and lmax >= 2 and ((ls[3] == 0 and max(ls[0], ls[1]) <= 3) or (ls[1] == 0 and max(ls[2], ls[3]) <= 3)):
-                    cands = cands + ["eri3s"]            # (ab|c s) / (a s|cd): the one-warp kernel with a two-centre ket
+                if not three and lmax >= 2 and e3_serves(ls):
+                    cands = cands + ["eri3s"]            # the one-warp kernel with a two-centre ket (csrc/eri3s_inst.cu: eri3s_has_class)
                 dw = engine.DeviceWorkload(w); out = dw.alloc_out(True)
                 best = None
                 seen = set()

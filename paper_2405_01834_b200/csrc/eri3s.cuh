@@ -21,7 +21,7 @@ struct Eri3sArgs {
     ShellView X;                          // the one-centre ket shell, or shell c of a two-centre ket (c, s)
     ShellView D;                          // two-centre ket: its s shell d
     const int32_t *kidx;                  // two-centre ket: pair list (c, d) or nullptr
-    int KD, swap;                         // swap = 1: the kernel's bra is the CALLER's ket (index columns and output strides swapped)
+    int KD, lD, swap;                     // lD: angular momentum of d (two-centre ket); swap = 1: the kernel's bra is the CALLER's ket (index columns and output strides swapped)
     long long s_t, s_ab, s_c;             // output strides (doubles) of the triplet / quartet, the ab block index, the c index
     int pure, la, lb, lX, Ka, Kb, KX;
     int nca, ncb, nXc, nhb, L;            // Cartesian counts of a, b; components of X in the result; N~(la+lb); la+lb+lX
@@ -37,9 +37,9 @@ struct Eri3sArgs {
 // NXC = components of X in the result (2 lX + 1, or the Cartesian count), a compile-time constant so that the two hot loops
 // (Hobson G build, bra box loop) unroll exactly: with a run-time count every multiply-add carried a compare and its own
 // 8-byte shared-memory load (34 % + 28 % of the stall samples of (ff|f) K = 4, profiles/r02_eri3s.md).
-// MODE 0: one-centre solid X (Hobson form); 1: one-centre Cartesian X; 2: two-centre ket (c, s_d) of a 4-center class -- G is
-// built in the Cartesian components of c from the three 1-D tables of the pair (Eqs. 9, 10, 13: the s shell only moves the
-// centre and adds the exponential), and the solid transform of c (Eq. 16), if asked for, is a third pass at the end.
+// MODE 0: one-centre solid X (Hobson form); 1: one-centre Cartesian X; 2: two-centre ket (c, d) of a 4-center class -- G is
+// built in the Cartesian components (c, d) from the three 1-D tables of the ket pair (Eqs. 9, 10, 13), NXC = ncart(lc) ncart(ld)
+// columns, and the solid transforms of d and c (Eq. 16), if asked for, are two more passes at the end.
 template <int NXC, int MODE>
 __global__ void __launch_bounds__(256) eri3s_kernel(Eri3sArgs g) {
     constexpr bool PURE = MODE == 0, TWO = MODE == 2;
@@ -48,7 +48,7 @@ __global__ void __launch_bounds__(256) eri3s_kernel(Eri3sArgs g) {
     // CTA-wide constants: Hermite triples and the transposed Cartesian->solid tables of a, b, X
     uint32_t *s_herm = (uint32_t *)sm;                               // nherm(12) words
     double *CT = sm + 228;                                           // 4 x 28 x MD_HL_CSTR
-    const int ls[4] = {g.la, g.lb, g.lX, 0};
+    const int ls[4] = {g.la, g.lb, g.lX, MODE == 2 ? g.lD : 0};
     if (blockDim.x == 256) hl_stage_tables<256>(s_herm, nherm(g.L), CT, ls);
     else hl_stage_tables<128>(s_herm, nherm(g.L), CT, ls);
     const int CTS = 28 * MD_HL_CSTR;
@@ -68,10 +68,15 @@ __global__ void __launch_bounds__(256) eri3s_kernel(Eri3sArgs g) {
     const uint2 *lut = (const uint2 *)g.rlut;
     const int la = g.la, lb = g.lb, lX = g.lX, Lb = la + lb, L = g.L, nt = Lb + 1;
     constexpr int nXc = NXC;
+    // columns a lane keeps in registers per pass of the bra box loop: all of them up to 12, else a divisor, else 7
+    constexpr int CW = nXc <= 12 ? nXc : nXc % 12 == 0 ? 12 : nXc % 10 == 0 ? 10 : nXc % 9 == 0 ? 9 : nXc == 15 ? 8 : 7;
     const int nca = g.nca, ncb = g.ncb, nhb = g.nhb, nab_c = nca * ncb;
     const int esz = (la + 1) * (lb + 1) * nt;
     const uint32_t *ca = s_herm + nherm(la - 1), *cb = s_herm + nherm(lb - 1), *cx = s_herm + nherm(lX - 1);
     const int ncx = ncart(lX), nlow = nherm(lX - 1);
+    const int lD = TWO ? g.lD : 0, ncdd = ncart(lD), ntk = lX + lD + 1, eszk = (lX + 1) * (lD + 1) * ntk;   // ket pair tables E[(i (lD+1) + j) ntk + t]
+    const uint32_t *cdl = s_herm + nherm(lD - 1);
+    const double *CdT = CT + 3 * CTS;
     const long long wstride = (long long)gridDim.x * g.warps;
 
     for (long long t = (long long)blockIdx.x * g.warps + warp; t < g.nt; t += wstride) {
@@ -125,9 +130,9 @@ __global__ void __launch_bounds__(256) eri3s_kernel(Eri3sArgs g) {
                     G0[lane] = f;
                     if (lane == L) ((L & 1) ? R1 : R0)[0] = f;
                 }
-                if constexpr (TWO) {                                 // the pair (c, s): E^t_{i0} per axis, exponential included (Eq. 13)
+                if constexpr (TWO) {                                 // the ket pair: E^t_{ij} per axis, exponential included (Eq. 13)
 #pragma unroll
-                    for (int x = 0; x < 3; ++x) hl_e_axis_warp(lX, 0, zc, zd, Xc[x] - Dc[x], EX + x * (lX + 1) * (lX + 1), lane);
+                    for (int x = 0; x < 3; ++x) hl_e_axis_warp(lX, lD, zc, zd, Xc[x] - Dc[x], EX + x * eszk, lane);
                 } else if (!PURE) hl_e_axis_warp(lX, 0, zx, 0.0, 0.0, EX, lane);   // one-centre table (Eq. 8), the same on the three axes
                 __syncwarp();
                 for (int m = L - 1; m >= 0; --m) {                   // Eq. 24, level m from level m + 1
@@ -171,23 +176,25 @@ __global__ void __launch_bounds__(256) eri3s_kernel(Eri3sArgs g) {
 #pragma unroll
                         for (int m = 0; m < nXc; ++m) o[m] = fma(f, sacc[m], o[m]);
                     }
-                } else if constexpr (nXc <= 15) {
-                    // l_X <= 4: the dense table HX[q~][c] = (-1)^{|q~|} E^t_{cx} E^u_{cy} E^v_{cz} of this ket primitive (Eqs. 7, 8, 19;
-                    // zero where a Hermite index exceeds the Cartesian one), then lane = p~ with every column in registers: three
-                    // times the multiply-adds of the sparse walk below, but no per-element box loop and no divergence
-                    const int ntx = lX + 1, nhx = nherm(lX), exsz = (TWO ? 3 : 1) * ntx * ntx;
-                    const double *EY = TWO ? EX + ntx * ntx : EX, *EZ = TWO ? EX + 2 * ntx * ntx : EX;
+                } else if constexpr (nXc <= 15 || (TWO && nXc != 21 && nXc != 28)) {
+                    // The dense table HX[q~][col] = (-1)^{|q~|} E^t E^u E^v of this ket primitive (Eqs. 7, 8, 19; zero where a Hermite
+                    // index exceeds the Cartesian sum), then lane = p~ with every column in registers: about three times the
+                    // multiply-adds of the sparse walk below, but no per-element box loop and no divergence.  col = c ncart(lD) + d.
+                    const int nhx = nherm(lX + lD), exsz = (TWO ? 3 : 1) * eszk;
+                    const double *EY = TWO ? EX + eszk : EX, *EZ = TWO ? EX + 2 * eszk : EX;
                     constexpr int NP = (nXc + 1) / 2, HS = 2 * NP;
                     double *HX = EX + exsz + (exsz & 1);
                     for (int i = lane; i < nhx * HS; i += 32) {
                         const int iq = i / HS, c = i - iq * HS;
                         double e3 = 0.0;
                         if (c < nXc) {
-                            int ex, ey, ez, t2, u2, v2;
-                            unpack_tuv(cx[c], ex, ey, ez);
+                            const int ci = c / ncdd, di = c - ci * ncdd;
+                            int ex, ey, ez, dx, dy, dz, t2, u2, v2;
+                            unpack_tuv(cx[ci], ex, ey, ez);
+                            unpack_tuv(cdl[di], dx, dy, dz);
                             unpack_tuv(s_herm[iq], t2, u2, v2);
-                            if (t2 <= ex && u2 <= ey && v2 <= ez) {
-                                e3 = EX[ex * ntx + t2] * EY[ey * ntx + u2] * EZ[ez * ntx + v2];
+                            if (t2 <= ex + dx && u2 <= ey + dy && v2 <= ez + dz) {
+                                e3 = EX[(ex * (lD + 1) + dx) * ntk + t2] * EY[(ey * (lD + 1) + dy) * ntk + u2] * EZ[(ez * (lD + 1) + dz) * ntk + v2];
                                 if ((t2 + u2 + v2) & 1) e3 = -e3;
                             }
                         }
@@ -247,10 +254,10 @@ __global__ void __launch_bounds__(256) eri3s_kernel(Eri3sArgs g) {
                 unpack_tuv(cb[b], bx, by, bz);
                 const double *ex = Ex + (ax * (lb + 1) + bx) * nt, *ey = Ey + (ay * (lb + 1) + by) * nt, *ez = Ez + (az * (lb + 1) + bz) * nt;
 #pragma unroll
-                for (int c0 = 0; c0 < nXc; c0 += 7) {
-                    double r[7];
+                for (int c0 = 0; c0 < nXc; c0 += CW) {
+                    double r[CW];
 #pragma unroll
-                    for (int c = 0; c < 7; ++c) r[c] = 0.0;
+                    for (int c = 0; c < CW; ++c) r[c] = 0.0;
                     // ONE flat loop over the lane's own box with per-lane counters: nested loops with lane-dependent bounds would
                     // make the warp walk the union of all boxes (84 steps for (ff|) instead of the largest one (27)
                     const int nx = ax + bx, ny = ay + by, nz = az + bz, box = (nx + 1) * (ny + 1) * (nz + 1);
@@ -259,13 +266,13 @@ __global__ void __launch_bounds__(256) eri3s_kernel(Eri3sArgs g) {
                         const double e3 = ex[tt] * ey[uu] * ez[vv];
                         const double *row = G + cube[(tt * nt + uu) * nt + vv] * nXc + c0;
 #pragma unroll
-                        for (int c = 0; c < 7; ++c)
+                        for (int c = 0; c < CW; ++c)
                             if (c0 + c < nXc) r[c] = fma(e3, row[c], r[c]);
                         if (++vv > nz) { vv = 0; if (++uu > ny) { uu = 0; ++tt; } }
                     }
                     double *o = acc + ab * nXc + c0;
 #pragma unroll
-                    for (int c = 0; c < 7; ++c)
+                    for (int c = 0; c < CW; ++c)
                         if (c0 + c < nXc) o[c] += r[c];
                 }
             }
@@ -317,15 +324,22 @@ __global__ void __launch_bounds__(256) eri3s_kernel(Eri3sArgs g) {
                         if (m < nsb) out[(ma * nsb + m) * g.s_ab + c * g.s_c] = oacc[m];
                 }
             }
-            if constexpr (TWO) {                                     // Eq. 16 on c
+            if constexpr (TWO) {                                     // Eq. 16 on d, then on c
                 __syncwarp();
-                const int nsx = nsolid(lX);
-                for (int i = lane; i < nsa * nsb * nsx; i += 32) {
-                    const int ab = i / nsx, m = i - ab * nsx;
+                const int nsx = nsolid(lX), nsd = nsolid(lD), nmab = nsa * nsb;
+                double *T2 = W;                                      // [ma mb][c][md] (the R / G region again)
+                for (int i = lane; i < nmab * ncx * nsd; i += 32) {
+                    const int md = i % nsd, r2 = i / nsd;            // r2 = mab ncx + c
                     double v = 0.0;
-#pragma unroll
-                    for (int c = 0; c < nXc; ++c) v = fma(CxT[c * MD_HL_CSTR + m], acc[ab * nXc + c], v);
-                    out[ab * g.s_ab + m * g.s_c] = v;
+                    for (int d = 0; d < ncdd; ++d) v = fma(CdT[d * MD_HL_CSTR + md], acc[r2 * ncdd + d], v);
+                    T2[i] = v;
+                }
+                __syncwarp();
+                for (int i = lane; i < nmab * nsx * nsd; i += 32) {
+                    const int md = i % nsd, r2 = i / nsd, mc = r2 % nsx, ab = r2 / nsx;
+                    double v = 0.0;
+                    for (int c = 0; c < ncx; ++c) v = fma(CxT[c * MD_HL_CSTR + mc], T2[(ab * ncx + c) * nsd + md], v);
+                    out[ab * g.s_ab + (mc * nsd + md) * g.s_c] = v;
                 }
             }
         }

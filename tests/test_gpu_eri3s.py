@@ -48,7 +48,11 @@ def test_eri3s_index_lists_and_product_mode():
 
 TWO = [((3, 2, 2, 0), (1, 1, 1, 1)), ((2, 1, 4, 0), (2, 1, 1, 2)), ((3, 3, 6, 0), (1, 1, 1, 1)), ((1, 0, 0, 0), (1, 2, 2, 1)),
        ((3, 3, 3, 0), (2, 2, 1, 3)), ((0, 0, 5, 0), (1, 1, 1, 1)),
-       ((3, 0, 2, 1), (1, 1, 1, 1)), ((5, 0, 3, 3), (1, 1, 1, 1)), ((4, 0, 1, 1), (2, 2, 1, 1)), ((6, 0, 3, 2), (1, 1, 2, 1))]
+       ((3, 0, 2, 1), (1, 1, 1, 1)), ((5, 0, 3, 3), (1, 1, 1, 1)), ((4, 0, 1, 1), (2, 2, 1, 1)), ((6, 0, 3, 2), (1, 1, 2, 1)),
+       # general two-centre kets (pp|, (dp|, (fp|, (dd| through the dense ket table, and their transposes
+       ((3, 2, 1, 1), (1, 1, 1, 1)), ((3, 3, 2, 1), (1, 1, 1, 1)), ((2, 1, 2, 2), (2, 1, 1, 2)), ((3, 3, 3, 1), (1, 1, 1, 1)),
+       ((1, 1, 3, 2), (1, 2, 1, 1)), ((0, 0, 2, 2), (1, 1, 1, 1)), ((3, 1, 1, 2), (1, 1, 2, 1)), ((2, 2, 3, 3), (1, 1, 1, 1)),
+       ((3, 3, 2, 2), (1, 1, 1, 1))]
 
 
 @pytest.mark.parametrize("ls,Ks", TWO, ids=[str(c[0]) for c in TWO])
