@@ -93,37 +93,7 @@ __device__ __forceinline__ int hl_herm_index(uint32_t w) {
     return ((n * (n + 1) * (n + 2) * 10923) >> 16) + ((a * (a + 1)) >> 1) + v;
 }
 
-// ---- S1: one Cartesian axis of the two-centre Hermite expansion, by one warp (lane = t) -----------------------------
-//   E^0_00 = exp(-za zb xab^2/p)                                              (Eq. 13)
-//   E^t_{i,j+1} = E^{t-1}_{ij}/(2p) + (P-B) E^t_{ij} + (t+1) E^{t+1}_{ij}     (Eq. 10), along i = 0
-//   E^t_{i+1,j} = E^{t-1}_{ij}/(2p) + (P-A) E^t_{ij} + (t+1) E^{t+1}_{ij}     (Eq. 9),  for every j
-// E[(i*(lb+1)+j)*nt + t], nt = la+lb+1 <= 13; entries with t > i+j are written as exact zeros (Eq. 14), which the
-// H build relies on.  A one-centre expansion (Eq. 8) is the case zb = 0, xab = 0.
-__device__ __forceinline__ void hl_e_axis_warp(int la, int lb, double za, double zb, double xab, double *E, int lane) {
-    const int nt = la + lb + 1;
-    const double p = za + zb, h = 0.5 / p;
-    const double xpa = -zb * xab / p, xpb = za * xab / p;
-    const double tp1 = (double)(lane + 1);
-    double e = lane == 0 ? exp(-za * zb / p * xab * xab) : 0.0;
-    if (lane < nt) E[lane] = e;
-    for (int j = 0; j < lb; ++j) {
-        double em = __shfl_up_sync(0xffffffffu, e, 1), ep = __shfl_down_sync(0xffffffffu, e, 1);
-        if (lane == 0) em = 0.0;
-        if (lane == 31) ep = 0.0;
-        e = xpb * e + h * em + tp1 * ep;
-        if (lane < nt) E[(j + 1) * nt + lane] = e;
-    }
-    for (int j = 0; j <= lb; ++j) {
-        e = lane < nt ? E[j * nt + lane] : 0.0;
-        for (int i = 0; i < la; ++i) {
-            double em = __shfl_up_sync(0xffffffffu, e, 1), ep = __shfl_down_sync(0xffffffffu, e, 1);
-            if (lane == 0) em = 0.0;
-            if (lane == 31) ep = 0.0;
-            e = xpa * e + h * em + tp1 * ep;
-            if (lane < nt) E[((i + 1) * (lb + 1) + j) * nt + lane] = e;
-        }
-    }
-}
+// hl_e_axis_warp (one Cartesian axis of the two-centre Hermite expansion by one warp) lives in common.cuh: pair.cuh uses it too.
 
 // Where H[p~][m] of one primitive pair goes in the CTA's scratch.
 struct HlBraDst {            // [kb*nhb + p~][sb]

@@ -18,39 +18,7 @@
 
 namespace mdb {
 
-// One Cartesian axis of the two-centre expansion, E[(i*(lb+1)+j)*nt + t], nt = la+lb+1:
-//   E^0_00 = exp(-za zb xab^2/p)                                        (Eq. 13)
-//   E^t_{i,j+1} = E^{t-1}_{ij}/(2p) + (P-B) E^t_{ij} + (t+1) E^{t+1}_{ij}   (Eq. 10), at i = 0
-//   E^t_{i+1,j} = E^{t-1}_{ij}/(2p) + (P-A) E^t_{ij} + (t+1) E^{t+1}_{ij}   (Eq. 9),  every j
-//   E^t_{ij} = 0 outside 0 <= t <= i+j                                  (Eq. 14)
-__device__ inline void hermite_e_axis(int la, int lb, double za, double zb, double xab, double *E) {
-    const int nt = la + lb + 1;
-    const double p = za + zb, h = 0.5 / p;
-    const double xpa = -zb * xab / p, xpb = za * xab / p;
-    for (int k = 0; k < (la + 1) * (lb + 1) * nt; ++k) E[k] = 0.0;
-    E[0] = exp(-za * zb / p * xab * xab);
-    for (int j = 0; j < lb; ++j) {                       // row i = 0: raise j
-        const double *src = E + j * nt;
-        double *dst = E + (j + 1) * nt;
-        for (int t = 0; t <= j + 1; ++t) {
-            double v = xpb * src[t];
-            if (t > 0) v += h * src[t - 1];
-            if (t < j) v += (t + 1) * src[t + 1];
-            dst[t] = v;
-        }
-    }
-    for (int i = 0; i < la; ++i)                         // raise i for every j
-        for (int j = 0; j <= lb; ++j) {
-            const double *src = E + (i * (lb + 1) + j) * nt;
-            double *dst = E + ((i + 1) * (lb + 1) + j) * nt;
-            for (int t = 0; t <= i + j + 1; ++t) {
-                double v = xpa * src[t];
-                if (t > 0) v += h * src[t - 1];
-                if (t < i + j) v += (t + 1) * src[t + 1];
-                dst[t] = v;
-            }
-        }
-}
+// The 1-D tables E[(i*(lb+1)+j)*nt + t], nt = la+lb+1 (Eqs. 9, 10, 13, 14) come from hl_e_axis_warp (common.cuh), one warp per axis.
 
 struct PairSetupArgs {
     PairView pv;
@@ -93,17 +61,19 @@ __global__ void __launch_bounds__(128) pair_setup_kernel(PairSetupArgs g) {
     long long ia = ipair, ib = ipair;
     if (pv.idx) { ia = pv.idx[2 * ipair]; ib = pv.idx[2 * ipair + 1]; }
 
-    if (threadIdx.x < 3) {
-        const int ax = threadIdx.x;
+    if (threadIdx.x < 96) {             // one WARP per Cartesian axis (lane = t, neighbours by shuffle): a single thread per axis
+        const int ax = threadIdx.x >> 5, lane = threadIdx.x & 31;   // took as long as the whole H build behind it ((ff|: 350 dependent DFMAs)
         double za = pv.a.exps[ia * Ka + ka], A = pv.a.center[3 * ia + ax];
         double zb = 0.0, B = A;
         if (!pv.single) { zb = pv.b.exps[ib * Kb + kb]; B = pv.b.center[3 * ib + ax]; }
-        hermite_e_axis(la, lb, za, zb, A - B, E + ax * esz);
-        double p = za + zb;
-        hdr[1 + ax] = (za * A + zb * B) / p;
-        if (ax == 0) {
-            hdr[0] = p;
-            hdr[4] = pv.a.coefs[ia * Ka + ka] * (pv.single ? 1.0 : pv.b.coefs[ib * Kb + kb]);
+        hl_e_axis_warp(la, lb, za, zb, A - B, E + ax * esz, lane);
+        if (lane == 0) {
+            double p = za + zb;
+            hdr[1 + ax] = (za * A + zb * B) / p;
+            if (ax == 0) {
+                hdr[0] = p;
+                hdr[4] = pv.a.coefs[ia * Ka + ka] * (pv.single ? 1.0 : pv.b.coefs[ib * Kb + kb]);
+            }
         }
     }
     __syncthreads();
