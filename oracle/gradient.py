@@ -13,11 +13,12 @@ themselves are oracle.eri4's; this module only writes the derivative rule out.
 
 Pins (tests/test_oracle_gradient.py): Richardson-extrapolated central differences of oracle.eri4 under a displaced centre
 (uses no derivative rule at all), translational invariance (the four centre derivatives sum to zero), the closed form of
-d/dA (ss|ss), and (ab|cd) symmetry of the derivative blocks.
+d/dA (ss|ss), and (ab|cd) symmetry of the derivative blocks; the 3-center form by the same finite differences of oracle.eri3,
+its three derivatives summing to zero, and agreement with the 4-center form on a zeta = 0 dummy shell.
 """
 import numpy as np
 
-from . import cart2solid, eri4, ncart
+from . import cart2solid, eri3, eri4, ncart
 
 
 def cart_components(l):
@@ -62,4 +63,36 @@ def eri4_grad(a, b, c, d, ia, ib, ic, id_, pure, center, quad=False):
     if pure:
         Ca, Cb, Cc, Cd = (cart2solid(s[0]) for s in shells)
         G = np.einsum("nxabcd,pa,qb,rc,sd->nxpqrs", G, Ca, Cb, Cc, Cd, optimize=True)
+    return G
+
+
+def eri3_grad(a, b, x, ia, ib, ix, pure, center, quad=False):
+    """d/dR_i (ab|X), R the centre of shell `center` (0, 1, 2 = a, b, X).  Returns out[n, 3, na, nb, nX].
+
+    The same rule on the 3-center integrals of oracle.eri3 (Eqs. 2, 6, 8)."""
+    shells = [a, b, x]
+    l, cen, ex, co = shells[center]
+    ex = np.asarray(ex, dtype=np.float64).reshape(np.asarray(cen).reshape(-1, 3).shape[0], -1)
+    co = np.asarray(co, dtype=np.float64).reshape(ex.shape)
+    idx = (ia, ib, ix)
+    up = list(shells)
+    up[center] = (l + 1, cen, ex, 2.0 * ex * co)
+    U = np.moveaxis(eri3(up[0], up[1], up[2], *idx, False, quad=quad), 1 + center, 1)
+    if l > 0:
+        dn = list(shells)
+        dn[center] = (l - 1, cen, ex, co)
+        Dn = np.moveaxis(eri3(dn[0], dn[1], dn[2], *idx, False, quad=quad), 1 + center, 1)
+    G = np.zeros((U.shape[0], 3, ncart(l)) + U.shape[2:])
+    for k, (ax, ay, az) in enumerate(cart_components(l)):
+        e = [ax, ay, az]
+        for i in range(3):
+            r = list(e); r[i] += 1
+            G[:, i, k] = U[:, cart_index(*r)]
+            if e[i] > 0:
+                s = list(e); s[i] -= 1
+                G[:, i, k] -= e[i] * Dn[:, cart_index(*s)]
+    G = np.moveaxis(G, 2, 2 + center)
+    if pure:
+        Ca, Cb, Cx = (cart2solid(s[0]) for s in shells)
+        G = np.einsum("nxabc,pa,qb,rc->nxpqr", G, Ca, Cb, Cx, optimize=True)
     return G

@@ -102,3 +102,49 @@ def test_component_order_helpers():
         comps = gradient.cart_components(l)
         assert len(comps) == oracle.ncart(l)
         assert [gradient.cart_index(*c) for c in comps] == list(range(len(comps)))
+
+
+# ---- 3-center (ab|X) ----------------------------------------------------------------------------------------------------------
+
+def fd_grad3(sh, idx, pure, center, h=2e-2):
+    out = []
+    for i in range(3):
+        def D(hh):
+            p = list(sh); m = list(sh)
+            p[center] = displaced(sh[center], i, hh)
+            m[center] = displaced(sh[center], i, -hh)
+            return (oracle.eri3(*p, *idx, pure) - oracle.eri3(*m, *idx, pure)) / (2 * hh)
+        out.append((4 * D(h / 2) - D(h)) / 3)
+    return np.stack(out, axis=1)
+
+
+CASES3 = [((0, 0, 0), (1, 1, 1)), ((1, 0, 2), (1, 2, 1)), ((2, 1, 1), (2, 1, 1)), ((2, 2, 3), (1, 1, 1)), ((3, 1, 4), (1, 1, 2)), ((0, 2, 5), (1, 1, 1))]
+
+
+@pytest.mark.parametrize("ls,Ks", CASES3, ids=[str(c[0]) for c in CASES3])
+@pytest.mark.parametrize("pure", [False, True])
+def test_gradient3_matches_finite_differences_and_sums_to_zero(ls, Ks, pure):
+    rng = np.random.default_rng(sum(ls) * 5 + pure)
+    sh = shells(rng, ls, Ks)
+    idx = [np.arange(3, dtype=np.int32)] * 3
+    gs = []
+    for center in range(3):
+        g = gradient.eri3_grad(*sh, *idx, pure, center)
+        f = fd_grad3(sh, idx, pure, center)
+        scale = np.abs(f).max()
+        assert np.abs(g - f).max() <= 2e-7 * scale, (center, np.abs(g - f).max() / scale)
+        gs.append(g)
+    assert np.abs(gs[0] + gs[1] + gs[2]).max() <= 1e-12 * max(np.abs(g).max() for g in gs)
+
+
+def test_gradient3_is_the_four_center_gradient_on_a_dummy_shell():
+    """(ab|X) = (ab|X s0) with a zeta = 0, c = 1 dummy (reading S7): the derivatives must agree."""
+    rng = np.random.default_rng(9)
+    sh = shells(rng, (2, 1, 3), (1, 2, 1))
+    dummy = (0, np.zeros((1, 3)), np.zeros((1, 1)), np.ones((1, 1)))
+    idx = [np.arange(3, dtype=np.int32)] * 3
+    z = np.zeros(3, dtype=np.int32)
+    for center in range(3):
+        g3 = gradient.eri3_grad(*sh, *idx, True, center)
+        g4 = gradient.eri4_grad(sh[0], sh[1], sh[2], dummy, idx[0], idx[1], idx[2], z, True, center)[..., 0]
+        assert np.allclose(g3, g4, rtol=1e-12, atol=1e-15)
