@@ -183,6 +183,10 @@ int md_exchange(const md_pairs *bra, const md_pairs *ket, int64_t nquartets, con
  */
 int md_eri4_grad(const md_pairs *bra, const md_pairs *ket, int64_t nquartets, const int32_t *quartet_idx, int pure,
                  int center, double *out, int64_t out_capacity_elems, void *cuda_stream);
+/* The same for (ab|X): center 0, 1, 2 = a, b, X (the three derivatives sum to zero); out[t][i][a][b][mX], 3 N_ab N_X doubles per
+ * triplet; arguments as md_eri3. */
+int md_eri3_grad(const md_pairs *bra, const md_shells *X, int64_t ntriplets, const int32_t *triplet_idx, int pure,
+                 int center, double *out, int64_t out_capacity_elems, void *cuda_stream);
 
 /* Number of doubles the result occupies (negative error code on bad arguments). */
 int64_t md_eri4_out_elems(int la, int lb, int lc, int ld, int pure, int64_t nquartets);

@@ -31,7 +31,7 @@ class md_pairs(ctypes.Structure):
 SYMBOLS = ["md_eri4", "md_eri3", "md_eri4_host", "md_eri3_host", "md_eri4_out_elems", "md_eri3_out_elems",
            "md_eri4_workspace_bytes", "md_eri3_workspace_bytes", "md_set_workspace", "md_set_variant",
            "md_last_variant", "md_last_launch_count", "md_init", "md_boys", "md_fp64_peak", "md_strerror", "md_last_cuda_error",
-           "md_version", "md_schwarz", "md_quartet_list", "md_exchange", "md_eri2", "md_eri4_static", "md_eri4_static_bytes", "md_eri4_grad"]
+           "md_version", "md_schwarz", "md_quartet_list", "md_exchange", "md_eri2", "md_eri4_static", "md_eri4_static_bytes", "md_eri4_grad", "md_eri3_grad"]
 
 _lib = None
 
@@ -59,6 +59,9 @@ def lib():
         L.md_eri4_grad.argtypes = [pp, pp, ctypes.c_int64, ctypes.c_void_p, ctypes.c_int, ctypes.c_int, ctypes.c_void_p,
                                    ctypes.c_int64, ctypes.c_void_p]
         L.md_eri4_grad.restype = ctypes.c_int
+        L.md_eri3_grad.argtypes = [pp, ps, ctypes.c_int64, ctypes.c_void_p, ctypes.c_int, ctypes.c_int, ctypes.c_void_p,
+                                   ctypes.c_int64, ctypes.c_void_p]
+        L.md_eri3_grad.restype = ctypes.c_int
         L.md_eri4_static_bytes.argtypes = [pp, pp, ctypes.c_int]
         L.md_eri4_static_bytes.restype = ctypes.c_int64
         L.md_eri4_workspace_bytes.argtypes = [pp, pp, ctypes.c_int64, ctypes.c_int, ctypes.c_int]
@@ -221,6 +224,15 @@ def md_eri4_grad(a, b, c, d, bra_idx, ket_idx, quartet_idx, nquartets, pure, cen
     bra = _pairs_struct(a, b, bra_idx, nbra)
     ket = _pairs_struct(c, d, ket_idx, nket)
     _check(lib().md_eri4_grad(ctypes.byref(bra), ctypes.byref(ket), int(nquartets), _ptr(quartet_idx), int(pure), int(center),
+                              _ptr(out), out.numel(), _stream_ptr(stream)))
+    return out
+
+
+def md_eri3_grad(a, b, x, bra_idx, triplet_idx, ntriplets, pure, center, out, stream=None, nbra=None):
+    """d/dR_i (ab|X) for the centre of shell `center` (0, 1, 2 = a, b, X): out[t][i][a][b][mX] on the DEVICE.  Asynchronous."""
+    bra = _pairs_struct(a, b, bra_idx, nbra)
+    xs = _shells_struct(x)
+    _check(lib().md_eri3_grad(ctypes.byref(bra), ctypes.byref(xs), int(ntriplets), _ptr(triplet_idx), int(pure), int(center),
                               _ptr(out), out.numel(), _stream_ptr(stream)))
     return out
 

@@ -68,3 +68,41 @@ def test_gradient_rejects_what_it_cannot_serve():
     engine.md_eri4_grad(dw.a, dw.b, dw.c, dw.d, None, None, dw.quartet_idx, 2, True, 1, out)   # the s shell of the same quartets is fine
     torch.cuda.synchronize()
     assert torch.isfinite(out).all()
+
+
+# ---- 3-center (ab|X) ----------------------------------------------------------------------------------------------------------
+
+def oracle_grad3(w, pure, center):
+    ia, ib, ic, _ = w.shell_indices(np.arange(w.nquartets))
+    sh = [(s.l, s.center, s.exps, s.coefs) for s in (w.a, w.b, w.c)]
+    return gradient.eri3_grad(*sh, ia, ib, ic, pure, center).reshape(w.nquartets, -1)
+
+
+def gpu_grad3(w, pure, center):
+    dw = engine.DeviceWorkload(w)
+    out = torch.full((w.nquartets * 3 * w.nout(pure),), float("nan"), dtype=torch.float64, device="cuda")
+    engine.md_eri3_grad(dw.a, dw.b, dw.c, dw.bra_idx, dw.quartet_idx, w.nquartets, pure, center, out, nbra=w.nbra)
+    torch.cuda.synchronize()
+    return out.cpu().numpy().reshape(w.nquartets, -1)
+
+
+CASES3 = [((0, 0, 0), (1, 1, 1), 67), ((1, 1, 1), (2, 1, 2), 67), ((2, 1, 3), (1, 2, 1), 41), ((3, 3, 2), (1, 1, 1), 23), ((2, 2, 5), (1, 1, 1), 19),
+          ((4, 1, 4), (1, 1, 1), 9), ((5, 5, 3), (1, 1, 1), 3)]
+
+
+@pytest.mark.parametrize("ls,Ks,n", CASES3, ids=[str(c[0]) for c in CASES3])
+@pytest.mark.parametrize("pure", [False, True])
+def test_gradient3_parity_every_centre(ls, Ks, n, pure):
+    w = W.independent_quartets("grad3", ls, Ks, n, (0.3, 6.0), (-2.0, 2.0), sum(ls) + 31, three_center=True)
+    got = []
+    for center in range(3):
+        g = gpu_grad3(w, pure, center)
+        assert_parity(g, oracle_grad3(w, pure, center), f"{ls} centre {center} pure={pure}")
+        got.append(g)
+    assert np.abs(got[0] + got[1] + got[2]).max() <= 1e-11 * max(np.abs(g).max() for g in got)
+
+
+def test_gradient3_product_mode():
+    w = W.product_batch("grad3p", (2, 1, 3), (1, 2, 1), 6, 5, (0.3, 6.0), (-2.0, 2.0), 8, three_center=True)
+    for center in range(3):
+        assert_parity(gpu_grad3(w, True, center), oracle_grad3(w, True, center), f"3-center product, centre {center}")
