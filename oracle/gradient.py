@@ -96,3 +96,14 @@ def eri3_grad(a, b, x, ia, ib, ix, pure, center, quad=False):
         Ca, Cb, Cx = (cart2solid(s[0]) for s in shells)
         G = np.einsum("nxabc,pa,qb,rc->nxpqr", G, Ca, Cb, Cx, optimize=True)
     return G
+
+
+def eri2_grad(x, y, ix, iy, pure, center, quad=False):
+    """d/dR_i (X|Y), R the centre of X (center 0) or Y (center 1).  Returns out[n, 3, nX, nY].
+
+    (X|Y) is the 4-center integral with a zeta = 0, c = 1 dummy s shell beside each of X and Y (oracle/two_center.py), so its
+    derivative is eri4_grad's with respect to position 0 or 2."""
+    dummy = (0, np.zeros((1, 3)), np.zeros((1, 1)), np.ones((1, 1)))
+    z = np.zeros(len(ix), dtype=np.int32)
+    g = eri4_grad(x, dummy, y, dummy, ix, z, iy, z, pure, 0 if center == 0 else 2, quad=quad)
+    return g[:, :, :, 0, :, 0]

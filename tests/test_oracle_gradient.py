@@ -148,3 +148,29 @@ def test_gradient3_is_the_four_center_gradient_on_a_dummy_shell():
         g3 = gradient.eri3_grad(*sh, *idx, True, center)
         g4 = gradient.eri4_grad(sh[0], sh[1], sh[2], dummy, idx[0], idx[1], idx[2], z, True, center)[..., 0]
         assert np.allclose(g3, g4, rtol=1e-12, atol=1e-15)
+
+
+# ---- 2-center (X|Y) -----------------------------------------------------------------------------------------------------------
+
+@pytest.mark.parametrize("lx,ly", [(0, 0), (1, 0), (2, 1), (3, 3), (0, 4), (5, 2)])
+@pytest.mark.parametrize("pure", [False, True])
+def test_gradient2_matches_finite_differences_of_the_two_center_oracle(lx, ly, pure):
+    from oracle import two_center
+    rng = np.random.default_rng(lx * 7 + ly + pure)
+    sh = shells(rng, (lx, ly), (2, 1))
+    ix = iy = np.arange(3, dtype=np.int32)
+    gs = []
+    for center in range(2):
+        g = gradient.eri2_grad(sh[0], sh[1], ix, iy, pure, center)
+        fd = []
+        for i in range(3):
+            def D(hh):
+                p = list(sh); m = list(sh)
+                p[center] = displaced(sh[center], i, hh)
+                m[center] = displaced(sh[center], i, -hh)
+                return (two_center.eri2(p[0], p[1], ix, iy, pure) - two_center.eri2(m[0], m[1], ix, iy, pure)) / (2 * hh)
+            fd.append((4 * D(1e-2) - D(2e-2)) / 3)
+        f = np.stack(fd, axis=1)
+        assert np.abs(g - f).max() <= 2e-7 * np.abs(f).max()
+        gs.append(g)
+    assert np.abs(gs[0] + gs[1]).max() <= 1e-12 * np.abs(gs[0]).max()      # the integral depends on X - Y only
