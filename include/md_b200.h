@@ -187,6 +187,10 @@ int md_eri4_grad(const md_pairs *bra, const md_pairs *ket, int64_t nquartets, co
  * triplet; arguments as md_eri3. */
 int md_eri3_grad(const md_pairs *bra, const md_shells *X, int64_t ntriplets, const int32_t *triplet_idx, int pure,
                  int center, double *out, int64_t out_capacity_elems, void *cuda_stream);
+/* The same for the 2-center (X|Y): center 0 = X, 1 = Y (the two derivatives are opposite); out[t][i][mX][mY]; arguments as md_eri2
+ * (MD_LAYOUT_QUARTET_MAJOR). */
+int md_eri2_grad(const md_shells *X, const md_shells *Y, int64_t npairs, const int32_t *pair_idx, int pure, int center,
+                 double *out, int64_t out_capacity_elems, void *cuda_stream);
 
 /* Number of doubles the result occupies (negative error code on bad arguments). */
 int64_t md_eri4_out_elems(int la, int lb, int lc, int ld, int pure, int64_t nquartets);

@@ -610,16 +610,19 @@ __global__ void __launch_bounds__(256) grad_solid_kernel(const double *__restric
     }
 }
 
-// ket != nullptr: (ab|cd), centres 0..3; X != nullptr: (ab|X), centres 0..2 (the fourth shell is then a one-component dummy).
-int run_grad(const md_pairs *bra, const md_pairs *ket, const md_shells *X, long long nq, const int32_t *qidx, int pure, int center,
-             double *out, long long cap, cudaStream_t st) {
-    if (center < 0 || center > (ket ? 3 : 2) || (pure != 0 && pure != 1) || nq < 0) return MD_EINVAL;
+// ket != nullptr: (ab|cd), centres 0..3; X != nullptr: (ab|X), centres 0..2 (the fourth shell is then a one-component dummy);
+// W != nullptr (and bra == ket == nullptr): the 2-center (W|X), centres 0 and 2 (dummies in positions 1 and 3).
+int md_eri2_impl(const md_shells *X, const md_shells *Y, int64_t npairs, const int32_t *pair_idx, int pure, int layout, double *out,
+                 int64_t out_capacity_elems, void *cuda_stream);
+int run_grad(const md_pairs *bra, const md_pairs *ket, const md_shells *X, const md_shells *W, long long nq, const int32_t *qidx, int pure,
+             int center, double *out, long long cap, cudaStream_t st) {
+    if (center < 0 || center > (ket ? 3 : 2) || (W && center == 1) || (pure != 0 && pure != 1) || nq < 0) return MD_EINVAL;
     md_shells dummy{};                                            // l = 0: one component, identity transform
-    const md_shells *sh[4] = {&bra->a, &bra->b, ket ? &ket->a : X, ket ? &ket->b : &dummy};
-    const long long nketp = ket ? ket->npairs : X->n;
+    const md_shells *sh[4] = {W ? W : &bra->a, W ? &dummy : &bra->b, ket ? &ket->a : X, ket ? &ket->b : &dummy};
+    const long long nbrap = W ? W->n : bra->npairs, nketp = ket ? ket->npairs : X->n;
     const int l = sh[center]->l;
     if (l + 1 > MD_MAX_L) return MD_EINVAL;                       // the raised shell must be one the kernels serve
-    if (!qidx && nq != bra->npairs * nketp) return MD_EINVAL;
+    if (!qidx && nq != nbrap * nketp) return MD_EINVAL;
     long long pc = 1, po = 1;                                     // Cartesian / output components of one quartet block
     for (int s = 0; s < 4; ++s) { pc *= ncart(sh[s]->l); po *= ncomp(sh[s]->l, pure); }
     if (3 * po * nq > cap) return MD_ECAPACITY;
@@ -633,10 +636,11 @@ int run_grad(const md_pairs *bra, const md_pairs *ket, const md_shells *X, long 
     for (int s = center + 1; s < 4; ++s) post *= ncart(sh[s]->l);
     const long long perU = pc / ncart(l) * ncart(l + 1), perD = l > 0 ? pc / ncart(l) * ncart(l - 1) : 0, perG = 3 * pc;
     // raised and lowered shell batches: same centres and exponents
-    md_pairs up[2] = {*bra, ket ? *ket : *bra}, dn[2] = {*bra, ket ? *ket : *bra};
-    md_shells Xu = X ? *X : dummy, Xd = Xu;
-    md_shells *su = center < 2 ? (center == 0 ? &up[0].a : &up[0].b) : !ket ? &Xu : (center == 2 ? &up[1].a : &up[1].b);
-    md_shells *sd = center < 2 ? (center == 0 ? &dn[0].a : &dn[0].b) : !ket ? &Xd : (center == 2 ? &dn[1].a : &dn[1].b);
+    md_pairs pz{};
+    md_pairs up[2] = {bra ? *bra : pz, ket ? *ket : pz}, dn[2] = {up[0], up[1]};
+    md_shells Xu = X ? *X : dummy, Xd = Xu, Wu = W ? *W : dummy, Wd = Wu;
+    md_shells *su = center < 2 ? (W ? &Wu : center == 0 ? &up[0].a : &up[0].b) : !ket ? &Xu : (center == 2 ? &up[1].a : &up[1].b);
+    md_shells *sd = center < 2 ? (W ? &Wd : center == 0 ? &dn[0].a : &dn[0].b) : !ket ? &Xd : (center == 2 ? &dn[1].a : &dn[1].b);
     const long long ncoef = (long long)sh[center]->n * sh[center]->K;
     size_t budget = (size_t)64 << 20;
     if (const char *env = getenv("MD_GRAD_CHUNK_BYTES")) budget = (size_t)atoll(env);
@@ -658,10 +662,12 @@ int run_grad(const md_pairs *bra, const md_pairs *ket, const md_shells *X, long 
         const long long m = std::min(chunk, nq - q0);
         const int32_t *qi = qidx ? qidx + 2 * q0 : ci;
         if (!qidx) { product_idx_kernel<<<(unsigned)((m + 255) / 256), 256, 0, st>>>(ci, q0, m, nketp); ++launches; }
-        e = run_call(view(up[0]), ket ? view(up[1]) : view_single(Xu), m, qi, 0, MD_LAYOUT_QUARTET_MAJOR, U, m * perU, st);
+        e = W ? md_eri2_impl(&Wu, &Xu, m, qi, 0, MD_LAYOUT_QUARTET_MAJOR, U, m * perU, st)
+              : run_call(view(up[0]), ket ? view(up[1]) : view_single(Xu), m, qi, 0, MD_LAYOUT_QUARTET_MAJOR, U, m * perU, st);
         launches += S.last_launches;
         if (e == MD_OK && l > 0) {
-            e = run_call(view(dn[0]), ket ? view(dn[1]) : view_single(Xd), m, qi, 0, MD_LAYOUT_QUARTET_MAJOR, Dn, m * perD, st);
+            e = W ? md_eri2_impl(&Wd, &Xd, m, qi, 0, MD_LAYOUT_QUARTET_MAJOR, Dn, m * perD, st)
+                  : run_call(view(dn[0]), ket ? view(dn[1]) : view_single(Xd), m, qi, 0, MD_LAYOUT_QUARTET_MAJOR, Dn, m * perD, st);
             launches += S.last_launches;
         }
         if (e != MD_OK) break;
@@ -800,7 +806,7 @@ int md_eri4_grad(const md_pairs *bra, const md_pairs *ket, int64_t nquartets, co
     int e = check_pairs(bra);
     if (e) return e;
     if ((e = check_pairs(ket))) return e;
-    return run_grad(bra, ket, nullptr, nquartets, quartet_idx, pure, center, out, out_capacity_elems, (cudaStream_t)cuda_stream);
+    return run_grad(bra, ket, nullptr, nullptr, nquartets, quartet_idx, pure, center, out, out_capacity_elems, (cudaStream_t)cuda_stream);
 }
 
 int md_eri3_grad(const md_pairs *bra, const md_shells *X, int64_t ntriplets, const int32_t *triplet_idx, int pure, int center,
@@ -808,7 +814,16 @@ int md_eri3_grad(const md_pairs *bra, const md_shells *X, int64_t ntriplets, con
     int e = check_pairs(bra);
     if (e) return e;
     if ((e = check_shells(X))) return e;
-    return run_grad(bra, nullptr, X, ntriplets, triplet_idx, pure, center, out, out_capacity_elems, (cudaStream_t)cuda_stream);
+    return run_grad(bra, nullptr, X, nullptr, ntriplets, triplet_idx, pure, center, out, out_capacity_elems, (cudaStream_t)cuda_stream);
+}
+
+int md_eri2_grad(const md_shells *X, const md_shells *Y, int64_t npairs, const int32_t *pair_idx, int pure, int center, double *out,
+                 int64_t out_capacity_elems, void *cuda_stream) {
+    int e = check_shells(X);
+    if (e) return e;
+    if ((e = check_shells(Y))) return e;
+    if (center != 0 && center != 1) return MD_EINVAL;
+    return run_grad(nullptr, nullptr, Y, X, npairs, pair_idx, pure, center == 0 ? 0 : 2, out, out_capacity_elems, (cudaStream_t)cuda_stream);
 }
 
 int md_exchange(const md_pairs *bra, const md_pairs *ket, int64_t nquartets, const int32_t *quartet_idx, int pure,
@@ -826,6 +841,14 @@ int md_exchange(const md_pairs *bra, const md_pairs *ket, int64_t nquartets, con
 
 int md_eri2(const md_shells *X, const md_shells *Y, int64_t npairs, const int32_t *pair_idx, int pure, int layout,
             double *out, int64_t out_capacity_elems, void *cuda_stream) {
+    return md_eri2_impl(X, Y, npairs, pair_idx, pure, layout, out, out_capacity_elems, cuda_stream);
+}
+
+}  // extern "C"
+
+namespace {
+int md_eri2_impl(const md_shells *X, const md_shells *Y, int64_t npairs, const int32_t *pair_idx, int pure, int layout,
+                 double *out, int64_t out_capacity_elems, void *cuda_stream) {
     int e = check_shells(X);
     if (e) return e;
     if ((e = check_shells(Y))) return e;
@@ -849,6 +872,9 @@ int md_eri2(const md_shells *X, const md_shells *Y, int64_t npairs, const int32_
     sc.release();
     return e;
 }
+}  // namespace
+
+extern "C" {
 
 int64_t md_eri4_out_elems(int la, int lb, int lc, int ld, int pure, int64_t n) {
     if (la < 0 || lb < 0 || lc < 0 || ld < 0 || la > MD_MAX_L || lb > MD_MAX_L || lc > MD_MAX_L || ld > MD_MAX_L ||

@@ -31,7 +31,7 @@ class md_pairs(ctypes.Structure):
 SYMBOLS = ["md_eri4", "md_eri3", "md_eri4_host", "md_eri3_host", "md_eri4_out_elems", "md_eri3_out_elems",
            "md_eri4_workspace_bytes", "md_eri3_workspace_bytes", "md_set_workspace", "md_set_variant",
            "md_last_variant", "md_last_launch_count", "md_init", "md_boys", "md_fp64_peak", "md_strerror", "md_last_cuda_error",
-           "md_version", "md_schwarz", "md_quartet_list", "md_exchange", "md_eri2", "md_eri4_static", "md_eri4_static_bytes", "md_eri4_grad", "md_eri3_grad"]
+           "md_version", "md_schwarz", "md_quartet_list", "md_exchange", "md_eri2", "md_eri4_static", "md_eri4_static_bytes", "md_eri4_grad", "md_eri3_grad", "md_eri2_grad"]
 
 _lib = None
 
@@ -62,6 +62,9 @@ def lib():
         L.md_eri3_grad.argtypes = [pp, ps, ctypes.c_int64, ctypes.c_void_p, ctypes.c_int, ctypes.c_int, ctypes.c_void_p,
                                    ctypes.c_int64, ctypes.c_void_p]
         L.md_eri3_grad.restype = ctypes.c_int
+        L.md_eri2_grad.argtypes = [ps, ps, ctypes.c_int64, ctypes.c_void_p, ctypes.c_int, ctypes.c_int, ctypes.c_void_p,
+                                   ctypes.c_int64, ctypes.c_void_p]
+        L.md_eri2_grad.restype = ctypes.c_int
         L.md_eri4_static_bytes.argtypes = [pp, pp, ctypes.c_int]
         L.md_eri4_static_bytes.restype = ctypes.c_int64
         L.md_eri4_workspace_bytes.argtypes = [pp, pp, ctypes.c_int64, ctypes.c_int, ctypes.c_int]
@@ -234,6 +237,14 @@ def md_eri3_grad(a, b, x, bra_idx, triplet_idx, ntriplets, pure, center, out, st
     xs = _shells_struct(x)
     _check(lib().md_eri3_grad(ctypes.byref(bra), ctypes.byref(xs), int(ntriplets), _ptr(triplet_idx), int(pure), int(center),
                               _ptr(out), out.numel(), _stream_ptr(stream)))
+    return out
+
+
+def md_eri2_grad(x, y, pair_idx, npairs, pure, center, out, stream=None):
+    """d/dR_i (X|Y) for the centre of X (center 0) or Y (1): out[t][i][mX][mY] on the DEVICE.  Asynchronous."""
+    xs, ys = _shells_struct(x), _shells_struct(y)
+    _check(lib().md_eri2_grad(ctypes.byref(xs), ctypes.byref(ys), int(npairs), _ptr(pair_idx), int(pure), int(center), _ptr(out),
+                              out.numel(), _stream_ptr(stream)))
     return out
 
 

@@ -106,3 +106,27 @@ def test_gradient3_product_mode():
     w = W.product_batch("grad3p", (2, 1, 3), (1, 2, 1), 6, 5, (0.3, 6.0), (-2.0, 2.0), 8, three_center=True)
     for center in range(3):
         assert_parity(gpu_grad3(w, True, center), oracle_grad3(w, True, center), f"3-center product, centre {center}")
+
+
+# ---- 2-center (X|Y) -----------------------------------------------------------------------------------------------------------
+
+@pytest.mark.parametrize("lx,ly", [(0, 0), (1, 0), (2, 1), (3, 3), (0, 4), (5, 2), (5, 5), (2, 6)])
+def test_gradient2_parity(lx, ly):
+    rng = np.random.default_rng(lx * 7 + ly)
+    x = W.make_shells(rng, 11, lx, 2, (0.3, 6.0), (-2.0, 2.0))
+    y = W.make_shells(rng, 9, ly, 1, (0.3, 6.0), (-2.0, 2.0))
+    pidx = np.stack([rng.integers(0, 11, 57), rng.integers(0, 9, 57)], 1).astype(np.int32)
+    dx, dy = engine.to_device(x), engine.to_device(y)
+    for pure in (True, False):
+        nout = engine.ncomp(lx, pure) * engine.ncomp(ly, pure)
+        for center in range(2):
+            if (lx if center == 0 else ly) > 5:
+                continue                                              # the raised shell would have l = 7
+            for idx in (pidx, None):
+                n = 57 if idx is not None else 99
+                out = torch.full((n * 3 * nout,), float("nan"), dtype=torch.float64, device="cuda")
+                engine.md_eri2_grad(dx, dy, engine.idx_to_device(idx), n, pure, center, out)
+                torch.cuda.synchronize()
+                ix, iy = (idx[:, 0], idx[:, 1]) if idx is not None else (np.repeat(np.arange(11), 9), np.tile(np.arange(9), 11))
+                ref = gradient.eri2_grad(x.astuple(), y.astuple(), ix.astype(np.int32), iy.astype(np.int32), pure, center)
+                assert_parity(out.cpu().numpy().reshape(n, -1), ref.reshape(n, -1), f"({lx}|{ly}) centre {center} pure={pure}")
