@@ -368,10 +368,11 @@ int run_rules(const PairView &b, const PairView &k, long long nq, const int32_t 
         }
     }
     // 3-center with la, lb <= 3 (BASELINE configs[2]): one warp per triplet in the sparse Cartesian form (eri3s.cuh); by
-    // measurement (profiles/r02_eri3s.md) under AUTO for every such class that has an l >= 2 shell.
+    // measurement (profiles/r02_autotune.csv) under AUTO when a shell has l >= 3 or la + lb >= 4; the smaller l <= 2 classes stay with `fused`
+    // ((ds|d) 0.097 against 0.379 ms per 100,000).
     // The same kernel serves 4-center classes with an s shell second in one pair, (ab|c s) or (a s|cd); those only when the
     // table (or the caller) names it.
-    if ((S.variant == MD_VARIANT_ERI3S || (S.variant == MD_VARIANT_AUTO && k.single && std::max({s.la, s.lb, s.lc}) >= 2)) &&
+    if ((S.variant == MD_VARIANT_ERI3S || (S.variant == MD_VARIANT_AUTO && k.single && (std::max({s.la, s.lb, s.lc}) >= 3 || s.la + s.lb >= 4))) &&
         layout == MD_LAYOUT_QUARTET_MAJOR && eri3s_has_class(b, k)) {
         if (sc.dry) { sc.need = 0; return MD_DRY; }
         if (eri3s_dispatch(b, k, nq, qidx, pure, out, S.boys_tab, fused_rlut(), S.nsm, st) == 1) {
